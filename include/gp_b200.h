@@ -1,0 +1,139 @@
+/*
+ * gp_b200.h -- C ABI of the B200-native (sm_100a, FP64) GP prediction pipeline of
+ * arxiv/paper_2602_19683 "GPU-Resident Gaussian Process Regression Leveraging Asynchronous
+ * Tasks with HPX".  Citations are PAPER.md:<line> (the text in /root/reference) and the
+ * readings A1..A12 listed in DESIGN.md.
+ *
+ * Conventions for every entry point
+ *   - All `d*` pointers are DEVICE pointers to FP64 (or int where stated), 16-byte aligned,
+ *     owned by the caller.  The library never frees or keeps caller memory.  Its only state is
+ *     a lazily built per-process cache of device-resident task schedules (a few MB, keyed by
+ *     problem shape) that gp_release_cached_schedules() drops.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every
+ *     call is stream-ordered and does not synchronise the host.
+ *   - Matrices are row-major, 0-based.  n = training points, m = test points
+ *     (n-hat in the paper), D = regressors per point, tile = tile edge t with
+ *     M = n/tile tiles per dimension.
+ *   - Tile sizes: tile > 0, tile % 32 == 0, n % tile == 0 and (where m is tiled) m % tile == 0;
+ *     anything else is GP_ERR_TILE (reading A7: the paper has no remainder case).
+ *   - Return value: GP_OK (0) or a negative GP_ERR_* reported synchronously before any work
+ *     is enqueued.  Numerical failure is reported through *d_info (see gp_cholesky_tiled).
+ *
+ * Tile layouts
+ *   GP_SYM_LOWER  lower-packed: only tiles (I,J) with J <= I are stored,
+ *                 tile (I,J) starts at ((I*(I+1)/2 + J) * tile*tile) doubles; element (r,c) of
+ *                 a tile is at r*tile + c.  Diagonal tiles are stored whole; after the
+ *                 factorisation their strict upper triangle is unspecified (reading A8).
+ *   GP_GENERAL    (na/tile) x (nb/tile) tiles, tile (a,b) at ((a*(nb/tile) + b) * tile*tile).
+ */
+#ifndef GP_B200_H_
+#define GP_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    GP_OK = 0,
+    GP_ERR_NULL = -1,        /* a required pointer is NULL */
+    GP_ERR_SIZE = -2,        /* n, m, na, nb or D <= 0, or beyond what the index arithmetic supports */
+    GP_ERR_TILE = -3,        /* tile <= 0, tile % 32 != 0, or a size not divisible by tile */
+    GP_ERR_HYPER = -4,       /* lengthscale <= 0, vertical <= 0, noise < 0, or non-finite */
+    GP_ERR_WORKSPACE = -5,   /* work_bytes smaller than gp_workspace_bytes() reports */
+    GP_ERR_CUDA = -6,        /* a CUDA runtime call failed (launch, memset, schedule upload) */
+    GP_ERR_MODE = -7         /* unknown layout mode */
+};
+
+enum { GP_SYM_LOWER = 0, GP_GENERAL = 1 };
+
+/* Hyperparameters of the squared-exponential kernel, PAPER.md:63 (Eq. 1) and PAPER.md:66:
+ *   k(xi,xj) = vertical * exp(-r2 / den) + delta_ij * noise,  r2 = sum_d (xi_d - xj_d)^2,
+ *   den = 2*lengthscale as printed in Eq. 1 (ell_squared == 0, the default), or
+ *   den = 2*lengthscale^2, the textbook form (ell_squared != 0) -- reading A1.
+ * The noise term is added ONLY on the diagonal of the training matrix K (reading A2). */
+typedef struct {
+    double lengthscale;
+    double vertical;
+    double noise;
+    int ell_squared;
+} gp_hyper;
+
+/* Covariance assembly in tiles -- PAPER.md:68 ("assemble multiple covariance matrices where each
+ * entry (i,j) corresponds to the kernel evaluation k(a_i, b_j)"), Eq. 1; steps a1/a9.
+ *   dA [na x D], dB [nb x D] row-major feature matrices.
+ *   mode GP_SYM_LOWER: requires dA == dB and na == nb; writes the M(M+1)/2 lower tiles of
+ *        K = K_{X,X} and adds h.noise on the global diagonal.
+ *   mode GP_GENERAL:   writes all (na/tile) x (nb/tile) tiles of K_{A,B}; never adds noise.
+ *   dTiles: output, (number of tiles) * tile^2 doubles in the layout above. */
+int gp_assemble_tiles(const double* dA, int64_t na, const double* dB, int64_t nb, int D, gp_hyper h,
+                      int tile, int mode, double* dTiles, void* stream);
+
+/* Tiled right-looking Cholesky K = L L^T, in place -- PAPER.md:83-139 (section 4.2, Fig. 1):
+ * POTRF on diagonal tiles, TRSM on panel tiles, SYRK / GEMM on trailing tiles (tile formulas per
+ * reading A3, loop nest per reading A4); steps a2-a6.
+ *   dKL: lower-packed tiles of K on entry, of L on exit (GP_SYM_LOWER layout).
+ *   sched_width: number of persistent worker CTAs that execute the tile-task DAG, the analogue
+ *        of the paper's CUDA-stream pool size; 0 = auto (one per SM).
+ *   d_info: device int. 0 = success; k > 0 = 1-based global column of the first non-positive
+ *        pivot (K not positive definite; reading A6).  After a failure the remaining tasks still
+ *        terminate and dKL is unspecified.
+ *   dWork/work_bytes: scratch, at least the `chol` size from gp_workspace_bytes(). On exit it
+ *        holds the inverted diagonal blocks of L that gp_predict_full_cov recomputes for itself,
+ *        so it may be freed or reused immediately. */
+int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork,
+                      size_t work_bytes, void* stream);
+
+/* Forward and backward substitution -- PAPER.md:72: L beta = y, then L^T alpha = beta; steps a7-a8.
+ *   dL: lower-packed tiles of L.  dY [n].  dAlpha [n] <- K^-1 y.
+ *   dBeta [n] <- L^-1 y; may be NULL, then dWork must hold n doubles more (see gp_workspace_bytes).
+ *   dWork/work_bytes: scratch, at least the `solve` size from gp_workspace_bytes(). */
+int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta,
+             void* dWork, size_t work_bytes, void* stream);
+
+/* Predictive mean -- PAPER.md:70 (Eq. 2) through PAPER.md:72: y^ = K_{X^,X} alpha; steps a9-a10.
+ * The cross-covariance is evaluated on the fly and never stored.
+ *   dX [n x D], dAlpha [n], dXs [m x D]; dMean [m] output.  No tiling constraint on n or m. */
+int gp_predict_mean(const double* dX, int64_t n, int D, const double* dAlpha, const double* dXs, int64_t m,
+                    gp_hyper h, double* dMean, void* stream);
+
+/* Full predictive covariance -- PAPER.md:76 (Eq. 3) computed as PAPER.md:79 prescribes:
+ * solve L V = K_{X,X^}, W = V^T V, Sigma = K_{X^,X^} - W; steps a9, a11, a12.
+ * V is held transposed (V^T = K_{X^,X} L^-T, m x n, GP_GENERAL tiles) in dWork.
+ *   dL: lower-packed tiles of L; dX [n x D]; dXs [m x D].
+ *   dSigma [m x m] dense row-major output; both triangles are written and are exactly symmetric.
+ *   sched_width as in gp_cholesky_tiled.
+ *   dWork/work_bytes: scratch, at least the `full_cov` size from gp_workspace_bytes(). */
+int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m,
+                        gp_hyper h, int tile, int sched_width, double* dSigma, void* dWork,
+                        size_t work_bytes, void* stream);
+
+/* Scratch sizes in bytes for the three calls that need scratch; any output pointer may be NULL.
+ * m may be 0 when only chol/solve are wanted. */
+int gp_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* chol, size_t* solve, size_t* full_cov);
+
+/* Unpack tiles to a dense row-major matrix (testing/inspection helper, not on the hot path).
+ *   lower_packed != 0: GP_SYM_LOWER tiles of an n x n matrix -> dDense [n x n] with the strict
+ *        upper triangle zeroed (reading A8);  nb is ignored.
+ *   lower_packed == 0: GP_GENERAL tiles of an n x nb matrix -> dDense [n x nb]. */
+int gp_tiles_to_dense(const double* dTiles, int64_t n, int64_t nb, int tile, int lower_packed,
+                      double* dDense, void* stream);
+
+/* Number of tile tasks (POTRF + TRSM + SYRK + GEMM) and of CTA-sized work items the scheduler
+ * runs for an n x n factorisation with this tile size (a6 bookkeeping; host only). */
+int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* work_items);
+
+/* Drop the cached device-resident schedules (synchronises the device). */
+void gp_release_cached_schedules(void);
+
+/* Size in doubles of the CTA-level block the tile tasks are split into for this tile size. */
+int gp_block_size(int tile);
+
+const char* gp_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GP_B200_H_ */

@@ -1,0 +1,220 @@
+"""Thin ctypes binding over libgp_b200.so (include/gp_b200.h): argument marshalling only.
+
+Every step of the pipeline runs in the library's CUDA kernels; PyTorch supplies device
+memory and the current stream.  There is NO CPU fallback: importing this module without the
+built library, or calling it without a CUDA device, raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgp_b200.so")
+
+GP_OK = 0
+GP_SYM_LOWER, GP_GENERAL = 0, 1
+ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA": -6, "MODE": -7}
+
+EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
+           "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
+           "gp_block_size", "gp_strerror")
+
+
+class gp_hyper(ctypes.Structure):
+    _fields_ = [("lengthscale", ctypes.c_double), ("vertical", ctypes.c_double), ("noise", ctypes.c_double),
+                ("ell_squared", ctypes.c_int)]
+
+
+@dataclass(frozen=True)
+class Hyper:
+    lengthscale: float = 1.0
+    vertical: float = 1.0
+    noise: float = 0.1
+    ell_squared: bool = False
+
+    def c(self) -> gp_hyper:
+        return gp_hyper(float(self.lengthscale), float(self.vertical), float(self.noise), int(bool(self.ell_squared)))
+
+
+class GpError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load the C-ABI library; fails loudly if it has not been built (python -m paper_2602_19683_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2602_19683_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_size_t
+    psz = ctypes.POINTER(ctypes.c_size_t)
+    lib.gp_assemble_tiles.argtypes = [vp, i64, vp, i64, ci, gp_hyper, ci, ci, vp, vp]
+    lib.gp_cholesky_tiled.argtypes = [vp, i64, ci, ci, vp, vp, sz, vp]
+    lib.gp_solve.argtypes = [vp, i64, ci, vp, vp, vp, vp, sz, vp]
+    lib.gp_predict_mean.argtypes = [vp, i64, ci, vp, vp, i64, gp_hyper, vp, vp]
+    lib.gp_predict_full_cov.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
+    lib.gp_workspace_bytes.argtypes = [i64, i64, ci, ci, psz, psz, psz]
+    lib.gp_tiles_to_dense.argtypes = [vp, i64, i64, ci, ci, vp, vp]
+    lib.gp_cholesky_task_counts.argtypes = [i64, ci, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.gp_release_cached_schedules.argtypes = []
+    lib.gp_release_cached_schedules.restype = None
+    lib.gp_block_size.argtypes = [ci]
+    lib.gp_strerror.argtypes = [ci]
+    lib.gp_strerror.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        if name not in ("gp_release_cached_schedules", "gp_strerror"):
+            getattr(lib, name).restype = ci
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load().gp_strerror(int(code)).decode()
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != GP_OK:
+        raise GpError(rc, where)
+
+
+def _ptr(t: torch.Tensor | None, dtype=torch.float64):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError("gp_b200 needs CUDA tensors (there is no CPU path)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"expected a contiguous {dtype} tensor, got {t.dtype} contiguous={t.is_contiguous()}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def num_lower_tiles(n: int, tile: int) -> int:
+    M = n // tile
+    return M * (M + 1) // 2
+
+
+def gp_block_size(tile: int) -> int:
+    return int(load().gp_block_size(int(tile)))
+
+
+def gp_workspace_bytes(n: int, m: int, D: int, tile: int):
+    c, s, f = ctypes.c_size_t(0), ctypes.c_size_t(0), ctypes.c_size_t(0)
+    _check(load().gp_workspace_bytes(n, m, D, tile, ctypes.byref(c), ctypes.byref(s), ctypes.byref(f)), "gp_workspace_bytes")
+    return int(c.value), int(s.value), int(f.value)
+
+
+def gp_cholesky_task_counts(n: int, tile: int):
+    a, b = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(load().gp_cholesky_task_counts(n, tile, ctypes.byref(a), ctypes.byref(b)), "gp_cholesky_task_counts")
+    return int(a.value), int(b.value)
+
+
+def gp_assemble_tiles(A: torch.Tensor, B: torch.Tensor, h: Hyper, tile: int, mode: int, out: torch.Tensor) -> torch.Tensor:
+    na, D = A.shape
+    nb = B.shape[0]
+    _check(load().gp_assemble_tiles(_ptr(A), na, _ptr(B), nb, D, h.c(), tile, mode, _ptr(out), _stream()), "gp_assemble_tiles")
+    return out
+
+
+def gp_cholesky_tiled(KL: torch.Tensor, n: int, tile: int, sched_width: int, info: torch.Tensor, work: torch.Tensor) -> None:
+    _check(load().gp_cholesky_tiled(_ptr(KL), n, tile, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8),
+                                    work.numel(), _stream()), "gp_cholesky_tiled")
+
+
+def gp_solve(L: torch.Tensor, n: int, tile: int, y: torch.Tensor, alpha: torch.Tensor, beta: torch.Tensor | None,
+             work: torch.Tensor) -> None:
+    _check(load().gp_solve(_ptr(L), n, tile, _ptr(y), _ptr(alpha), _ptr(beta), _ptr(work, torch.uint8), work.numel(), _stream()),
+           "gp_solve")
+
+
+def gp_predict_mean(X: torch.Tensor, alpha: torch.Tensor, Xs: torch.Tensor, h: Hyper, mean: torch.Tensor) -> None:
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_mean(_ptr(X), n, D, _ptr(alpha), _ptr(Xs), m, h.c(), _ptr(mean), _stream()), "gp_predict_mean")
+
+
+def gp_predict_full_cov(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
+                        Sigma: torch.Tensor, work: torch.Tensor) -> None:
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_full_cov(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(Sigma),
+                                      _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_full_cov")
+
+
+def gp_tiles_to_dense(tiles: torch.Tensor, n: int, nb: int, tile: int, lower_packed: bool, dense: torch.Tensor) -> torch.Tensor:
+    _check(load().gp_tiles_to_dense(_ptr(tiles), n, nb, tile, int(lower_packed), _ptr(dense), _stream()), "gp_tiles_to_dense")
+    return dense
+
+
+def gp_release_cached_schedules() -> None:
+    load().gp_release_cached_schedules()
+
+
+# ------------------------------------------------------------------------------------------------
+# Convenience driver: the whole pipeline of PAPER.md section 4.1 on device tensors (allocation and
+# call sequencing only).
+# ------------------------------------------------------------------------------------------------
+@dataclass
+class GpResult:
+    L_tiles: torch.Tensor
+    alpha: torch.Tensor
+    beta: torch.Tensor
+    info: torch.Tensor
+    mean: torch.Tensor | None = None
+    Sigma: torch.Tensor | None = None
+
+
+class GpPipeline:
+    """Pre-allocates every device buffer for one (n, m, D, tile) shape so that run() only launches."""
+
+    def __init__(self, n: int, m: int, D: int, tile: int, h: Hyper, sched_width: int = 0, device="cuda"):
+        self.n, self.m, self.D, self.tile, self.h, self.width = n, m, D, tile, h, sched_width
+        dev = torch.device(device)
+        cb, sb, fb = gp_workspace_bytes(n, m, D, tile)
+        self.KL = torch.empty(num_lower_tiles(n, tile) * tile * tile, dtype=torch.float64, device=dev)
+        self.work = torch.empty(max(cb, sb, fb), dtype=torch.uint8, device=dev)
+        self.info = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.alpha = torch.empty(n, dtype=torch.float64, device=dev)
+        self.beta = torch.empty(n, dtype=torch.float64, device=dev)
+        self.mean = torch.empty(m, dtype=torch.float64, device=dev) if m > 0 else None
+        self.Sigma = torch.empty(m, m, dtype=torch.float64, device=dev) if m > 0 else None
+
+    def assemble(self, X):
+        gp_assemble_tiles(X, X, self.h, self.tile, GP_SYM_LOWER, self.KL)
+
+    def cholesky(self):
+        gp_cholesky_tiled(self.KL, self.n, self.tile, self.width, self.info, self.work)
+
+    def solve(self, y):
+        gp_solve(self.KL, self.n, self.tile, y, self.alpha, self.beta, self.work)
+
+    def predict(self, X, Xs, full_cov=True):
+        gp_predict_mean(X, self.alpha, Xs, self.h, self.mean)
+        if full_cov:
+            gp_predict_full_cov(self.KL, X, Xs, self.h, self.tile, self.width, self.Sigma, self.work)
+
+    def run(self, X, y, Xs, full_cov=True) -> GpResult:
+        self.assemble(X)
+        self.cholesky()
+        self.solve(y)
+        self.predict(X, Xs, full_cov)
+        return GpResult(self.KL, self.alpha, self.beta, self.info, self.mean, self.Sigma if full_cov else None)
+
+    def dense_L(self) -> torch.Tensor:
+        out = torch.empty(self.n, self.n, dtype=torch.float64, device=self.KL.device)
+        return gp_tiles_to_dense(self.KL, self.n, self.n, self.tile, True, out)

@@ -1,0 +1,408 @@
+// gp_api.cu -- C ABI of libgp_b200.so (include/gp_b200.h): argument validation, workspace
+// carving, host-side construction of the static tile-task schedule, kernel launches.
+// No library linear algebra (cuBLAS / cuSOLVER) is linked or called anywhere in this library.
+#include "../../include/gp_b200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <vector>
+
+#include "gp_exec.cuh"
+#include "gp_kernels.cuh"
+#include "gp_schedule.h"
+
+using namespace gpb;
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int pick_block(int tile) {
+    if (tile % 128 == 0) return 128;
+    if (tile % 64 == 0) return 64;
+    return 32;
+}
+
+bool hyper_ok(const gp_hyper& h) {
+    return std::isfinite(h.lengthscale) && std::isfinite(h.vertical) && std::isfinite(h.noise) && h.lengthscale > 0.0 &&
+           h.vertical > 0.0 && h.noise >= 0.0;
+}
+
+HyperDev to_dev(const gp_hyper& h) {
+    HyperDev d;
+    d.den = h.ell_squared ? 2.0 * h.lengthscale * h.lengthscale : 2.0 * h.lengthscale;
+    d.vertical = h.vertical;
+    d.noise = h.noise;
+    return d;
+}
+
+int tile_ok(int64_t n, int tile) {
+    if (tile <= 0 || tile % 32 != 0) return GP_ERR_TILE;
+    if (n % tile != 0) return GP_ERR_TILE;
+    return GP_OK;
+}
+
+int sm_count() {
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    }
+    return sms;
+}
+
+// ---- device-resident schedule cache ---------------------------------------------------------
+struct CachedSchedule {
+    Item* d_items = nullptr;
+    int nitems = 0;
+};
+std::mutex g_mu;
+std::map<std::tuple<int, int, int, int, int>, CachedSchedule> g_cache;   // (device, kind, M, Mm, nbt)
+
+int get_schedule(int kind, int M, int Mm, int nbt, int blk, int workers, CachedSchedule* out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto key = std::make_tuple(dev, kind, M, Mm, nbt);
+    auto it = g_cache.find(key);
+    if (it != g_cache.end()) { *out = it->second; return GP_OK; }
+    std::vector<SchedItem> items;
+    if (kind == 0) build_cholesky_schedule(M, nbt, workers, items, blk);
+    else build_predict_schedule(M, Mm, nbt, workers, items, blk);
+    static_assert(sizeof(SchedItem) == sizeof(Item), "schedule item layout");
+    CachedSchedule cs;
+    cs.nitems = (int)items.size();
+    if (cudaMalloc(&cs.d_items, items.size() * sizeof(Item) + 16) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpy(cs.d_items, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaFree(cs.d_items);
+        return GP_ERR_CUDA;
+    }
+    g_cache[key] = cs;
+    *out = cs;
+    return GP_OK;
+}
+
+template <int BLK>
+int launch_exec(const ExecParams& p, int workers, cudaStream_t st) {
+    static bool configured = false;
+    constexpr int smem = exec_smem_bytes<BLK>();
+    if (!configured) {
+        if (cudaFuncSetAttribute(exec_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
+        configured = true;
+    }
+    exec_kernel<BLK><<<workers, kThreads, smem, st>>>(p);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int launch_exec_any(int b, const ExecParams& p, int workers, cudaStream_t st) {
+    switch (b) {
+        case 128: return launch_exec<128>(p, workers, st);
+        case 64: return launch_exec<64>(p, workers, st);
+        default: return launch_exec<32>(p, workers, st);
+    }
+}
+
+template <int BLK>
+int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStream_t st) {
+    static bool configured = false;
+    constexpr int smem = BLK * (BLK + 1) * 8;
+    if (!configured) {
+        if (cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
+        configured = true;
+    }
+    trtri_diag_kernel<BLK><<<NB, kThreads, smem, st>>>(L, t, nbt, invD);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaStream_t st) {
+    switch (b) {
+        case 128: return launch_trtri<128>(L, t, t / 128, NB, invD, st);
+        case 64: return launch_trtri<64>(L, t, t / 64, NB, invD, st);
+        default: return launch_trtri<32>(L, t, t / 32, NB, invD, st);
+    }
+}
+
+int workers_for(int sched_width) {
+    const int sms = sm_count();
+    if (sched_width <= 0) return sms;
+    return sched_width < sms ? sched_width : sms;   // one resident CTA per SM: more cannot be co-resident
+}
+
+int launch_assemble(const double* dA, int64_t na, const double* dB, int64_t nb, int D, const HyperDev& h, int tile, int sym_lower,
+                    double* out, cudaStream_t st) {
+    const int64_t Ma = na / tile, Mb = nb / tile;
+    const int64_t ntiles = sym_lower ? Ma * (Ma + 1) / 2 : Ma * Mb;
+    const int sb = (tile + kAsmBlk - 1) / kAsmBlk;
+    if (ntiles * sb * sb > 2147483647LL) return GP_ERR_SIZE;
+    dim3 grid((unsigned)(ntiles * sb * sb));
+    const size_t smem = 2 * (size_t)kAsmMaxD * kAsmBlk * sizeof(double);
+    assemble_tiles_kernel<<<grid, 256, smem, st>>>(dA, dB, D, h, tile, (int)Mb, sym_lower, out);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+// workspace layouts ---------------------------------------------------------------------------
+struct CholWs { size_t ticket, verL, invD, total; };
+CholWs chol_ws(int64_t n, int b) {
+    const size_t NB = (size_t)(n / b);
+    CholWs w;
+    w.ticket = 0;
+    w.verL = 256;
+    w.invD = align_up(w.verL + NB * NB * sizeof(int), 256);
+    w.total = w.invD + NB * (size_t)b * b * sizeof(double);
+    return w;
+}
+struct SolveWs { size_t ticket, flags, beta, invD, total; };
+SolveWs solve_ws(int64_t n, int b) {
+    const size_t NB = (size_t)(n / b);
+    SolveWs w;
+    w.ticket = 0;
+    w.flags = 256;
+    w.beta = align_up(w.flags + 2 * NB * sizeof(int), 256);
+    w.invD = align_up(w.beta + (size_t)n * sizeof(double), 256);
+    w.total = w.invD + NB * (size_t)b * b * sizeof(double);
+    return w;
+}
+struct CovWs { size_t ticket, verV, verS, invD, Vt, total; };
+CovWs cov_ws(int64_t n, int64_t m, int b) {
+    const size_t NB = (size_t)(n / b), NBm = (size_t)(m / b);
+    CovWs w;
+    w.ticket = 0;
+    w.verV = 256;
+    w.verS = align_up(w.verV + NBm * NB * sizeof(int), 256);
+    w.invD = align_up(w.verS + NBm * NBm * sizeof(int), 256);
+    w.Vt = align_up(w.invD + NB * (size_t)b * b * sizeof(double), 256);
+    w.total = w.Vt + (size_t)m * (size_t)n * sizeof(double);
+    return w;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gp_block_size(int tile) {
+    if (tile <= 0 || tile % 32 != 0) return GP_ERR_TILE;
+    return pick_block(tile);
+}
+
+const char* gp_strerror(int code) {
+    switch (code) {
+        case GP_OK: return "ok";
+        case GP_ERR_NULL: return "required pointer is NULL";
+        case GP_ERR_SIZE: return "invalid size (n, m, na, nb or D)";
+        case GP_ERR_TILE: return "invalid tile size (must be a positive multiple of 32 dividing n and m)";
+        case GP_ERR_HYPER: return "invalid hyperparameters";
+        case GP_ERR_WORKSPACE: return "workspace too small";
+        case GP_ERR_CUDA: return "CUDA runtime error";
+        case GP_ERR_MODE: return "unknown layout mode";
+        default: return "unknown error code";
+    }
+}
+
+int gp_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* chol, size_t* solve, size_t* full_cov) {
+    if (n <= 0 || m < 0 || D <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m > 0 && m % tile != 0) return GP_ERR_TILE;
+    const int b = pick_block(tile);
+    if (chol) *chol = chol_ws(n, b).total;
+    if (solve) *solve = solve_ws(n, b).total;
+    if (full_cov) *full_cov = m > 0 ? cov_ws(n, m, b).total : 0;
+    return GP_OK;
+}
+
+int gp_assemble_tiles(const double* dA, int64_t na, const double* dB, int64_t nb, int D, gp_hyper h, int tile, int mode,
+                      double* dTiles, void* stream) {
+    if (!dA || !dB || !dTiles) return GP_ERR_NULL;
+    if (na <= 0 || nb <= 0 || D <= 0) return GP_ERR_SIZE;
+    if (mode != GP_SYM_LOWER && mode != GP_GENERAL) return GP_ERR_MODE;
+    int rc = tile_ok(na, tile);
+    if (rc != GP_OK) return rc;
+    rc = tile_ok(nb, tile);
+    if (rc != GP_OK) return rc;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    if (mode == GP_SYM_LOWER && (dA != dB || na != nb)) return GP_ERR_SIZE;
+    return launch_assemble(dA, na, dB, nb, D, to_dev(h), tile, mode == GP_SYM_LOWER ? 1 : 0, dTiles, (cudaStream_t)stream);
+}
+
+int gp_tiles_to_dense(const double* dTiles, int64_t n, int64_t nb, int tile, int lower_packed, double* dDense, void* stream) {
+    if (!dTiles || !dDense) return GP_ERR_NULL;
+    if (n <= 0) return GP_ERR_SIZE;
+    if (lower_packed) nb = n;
+    if (nb <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    rc = tile_ok(nb, tile);
+    if (rc != GP_OK) return rc;
+    tiles_to_dense_kernel<<<sm_count() * 8, 256, 0, (cudaStream_t)stream>>>(dTiles, n, nb, tile, lower_packed, dDense);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* work_items) {
+    if (n <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const int64_t M = n / tile;
+    if (tile_tasks) *tile_tasks = M + M * (M - 1) / 2 + M * (M - 1) / 2 + M * (M - 1) * (M - 2) / 6;
+    if (work_items) {
+        std::vector<SchedItem> items;
+        build_cholesky_schedule((int)M, tile / pick_block(tile), 148, items, pick_block(tile), nullptr, false);
+        *work_items = (int64_t)items.size();
+    }
+    return GP_OK;
+}
+
+int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes, void* stream) {
+    if (!dKL || !d_info || !dWork) return GP_ERR_NULL;
+    if (n <= 0 || n > (int64_t)1 << 22) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const int b = pick_block(tile);
+    const CholWs w = chol_ws(n, b);
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b);
+    const int workers = workers_for(sched_width);
+    CachedSchedule cs;
+    rc = get_schedule(0, M, 0, nbt, b, sm_count(), &cs);
+    if (rc != GP_OK) return rc;
+    char* ws = (char*)dWork;
+    if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;        // ticket + version counters
+    if (cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return GP_ERR_CUDA;
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = dKL;
+    p.invD = (double*)(ws + w.invD);
+    p.verL = (int*)(ws + w.verL);
+    p.items = cs.d_items;
+    p.nitems = cs.nitems;
+    p.ticket = (unsigned int*)(ws + w.ticket);
+    p.d_info = d_info;
+    p.t = tile;
+    p.nbt = nbt;
+    p.NB = NB;
+    p.Mt = M;
+    return launch_exec_any(b, p, workers, st);
+}
+
+int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta, void* dWork, size_t work_bytes,
+             void* stream) {
+    if (!dL || !dY || !dAlpha || !dWork) return GP_ERR_NULL;
+    if (n <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const int b = pick_block(tile);
+    const SolveWs w = solve_ws(n, b);
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int NB = (int)(n / b);
+    char* ws = (char*)dWork;
+    if (cudaMemsetAsync(ws, 0, w.beta, st) != cudaSuccess) return GP_ERR_CUDA;
+    double* invD = (double*)(ws + w.invD);
+    double* beta = dBeta ? dBeta : (double*)(ws + w.beta);
+    int* flags = (int*)(ws + w.flags);
+    unsigned int* ticket = (unsigned int*)(ws + w.ticket);
+    rc = launch_trtri_any(b, dL, tile, NB, invD, st);
+    if (rc != GP_OK) return rc;
+    switch (b) {
+        case 128:
+            forward_solve_kernel<128><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
+            backward_solve_kernel<128><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
+            break;
+        case 64:
+            forward_solve_kernel<64><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
+            backward_solve_kernel<64><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
+            break;
+        default:
+            forward_solve_kernel<32><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
+            backward_solve_kernel<32><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
+            break;
+    }
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_predict_mean(const double* dX, int64_t n, int D, const double* dAlpha, const double* dXs, int64_t m, gp_hyper h, double* dMean,
+                    void* stream) {
+    if (!dX || !dAlpha || !dXs || !dMean) return GP_ERR_NULL;
+    if (n <= 0 || m <= 0 || D <= 0 || D > 512) return GP_ERR_SIZE;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    const unsigned grid = (unsigned)((m + kMeanTM - 1) / kMeanTM);
+    const size_t smem = ((size_t)kMeanTM * D + (size_t)kMeanTM * 256) * sizeof(double);
+    predict_mean_kernel<<<grid, 256, smem, (cudaStream_t)stream>>>(dX, n, D, dAlpha, dXs, m, to_dev(h), dMean);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
+                        int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
+    if (!dL || !dX || !dXs || !dSigma || !dWork) return GP_ERR_NULL;
+    if (n <= 0 || m <= 0 || D <= 0 || n > (int64_t)1 << 22 || m > (int64_t)1 << 22) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    rc = tile_ok(m, tile);
+    if (rc != GP_OK) return rc;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    const int b = pick_block(tile);
+    const CovWs w = cov_ws(n, m, b);
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = (int)(n / tile), Mm = (int)(m / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
+    const int workers = workers_for(sched_width);
+    CachedSchedule cs;
+    rc = get_schedule(1, M, Mm, nbt, b, sm_count(), &cs);
+    if (rc != GP_OK) return rc;
+    char* ws = (char*)dWork;
+    const HyperDev hd = to_dev(h);
+    double* Vt = (double*)(ws + w.Vt);
+    double* invD = (double*)(ws + w.invD);
+    if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;
+    // a9: K_{X^,X} (m x n, noise-free) straight into the V^T buffer; prior K_{X^,X^} straight into Sigma
+    rc = launch_assemble(dXs, m, dX, n, D, hd, tile, 0, Vt, st);
+    if (rc != GP_OK) return rc;
+    {
+        // dense m x m = one "tile" of edge m
+        const int sb = (int)((m + kAsmBlk - 1) / kAsmBlk);
+        if ((int64_t)sb * sb > 2147483647LL) return GP_ERR_SIZE;
+        dim3 grid((unsigned)(sb * sb));
+        const size_t smem = 2 * (size_t)kAsmMaxD * kAsmBlk * sizeof(double);
+        assemble_tiles_kernel<<<grid, 256, smem, st>>>(dXs, dXs, D, hd, (int)m, 1, 0, dSigma);
+        if (cudaGetLastError() != cudaSuccess) return GP_ERR_CUDA;
+    }
+    rc = launch_trtri_any(b, dL, tile, NB, invD, st);
+    if (rc != GP_OK) return rc;
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = const_cast<double*>(dL);
+    p.Vt = Vt;
+    p.S = dSigma;
+    p.invD = invD;
+    p.verV = (int*)(ws + w.verV);
+    p.verS = (int*)(ws + w.verS);
+    p.items = cs.d_items;
+    p.nitems = cs.nitems;
+    p.ticket = (unsigned int*)(ws + w.ticket);
+    p.t = tile;
+    p.nbt = nbt;
+    p.NB = NB;
+    p.NBm = NBm;
+    p.Mt = M;
+    p.m = m;
+    p.L_final = 1;
+    rc = launch_exec_any(b, p, workers, st);
+    if (rc != GP_OK) return rc;
+    dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
+    mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+void gp_release_cached_schedules(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    cudaDeviceSynchronize();
+    for (auto& kv : g_cache) cudaFree(kv.second.d_items);
+    g_cache.clear();
+}
+
+}  // extern "C"

@@ -1,0 +1,352 @@
+// gp_kernels.cuh -- the HBM/ALU-bound kernels of the pipeline: fused covariance assembly
+// (a1, a9), tile unpacking, the two triangular solves for alpha (a7, a8) and the fused
+// cross-covariance + mean (a9, a10).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gpb {
+
+struct HyperDev {
+    double den;       // 2*ell (Eq. 1 as printed) or 2*ell^2 (reading A1)
+    double vertical;  // v
+    double noise;     // sigma^2
+};
+
+// k(a,b) without the noise term -- PAPER.md:63, Eq. 1.  r2 accumulated in index order with FMA.
+__device__ __forceinline__ double se_kernel(double r2, const HyperDev& h) { return h.vertical * exp(-r2 / h.den); }
+
+// ---------------------------------------------------------------------------------------------
+// Fused assembly: distance, exp, noise in one pass, one 64x64 output sub-block per CTA.
+// Each thread produces a 4x4 patch (rows ty+16i, columns 4tx..4tx+3): 32 B contiguous per row
+// per thread, a warp writes two full 512 B row segments per store pair -> fully coalesced.
+// 1-D grid: blockIdx.x = tile index * sub-blocks per tile + sub-block.
+// sym_lower: tile list is the lower-packed (I,J), J<=I; noise is added where global i == j.
+// ---------------------------------------------------------------------------------------------
+constexpr int kAsmBlk = 64;
+constexpr int kAsmMaxD = 32;   // features staged in shared memory per pass; larger D is processed in chunks
+
+__global__ void __launch_bounds__(256) assemble_tiles_kernel(const double* __restrict__ A, const double* __restrict__ B,
+                                                             int D, HyperDev h, int tile, int tiles_b /* tiles per row (general) */,
+                                                             int sym_lower, double* __restrict__ out) {
+    extern __shared__ __align__(16) double sm[];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    // tile coordinates
+    int I, J;
+    const int sb = (tile + kAsmBlk - 1) / kAsmBlk;
+    const int tidx = blockIdx.x / (sb * sb), sub = blockIdx.x % (sb * sb);
+    if (sym_lower) {
+        // invert tidx = I(I+1)/2 + J
+        I = (int)((sqrt(8.0 * (double)tidx + 1.0) - 1.0) * 0.5);
+        while ((int64_t)(I + 1) * (I + 2) / 2 <= tidx) ++I;
+        while ((int64_t)I * (I + 1) / 2 > tidx) --I;
+        J = tidx - (int)((int64_t)I * (I + 1) / 2);
+    } else {
+        I = tidx / tiles_b;
+        J = tidx % tiles_b;
+    }
+    const int r0 = (sub / sb) * kAsmBlk, c0 = (sub % sb) * kAsmBlk;   // inside the tile
+    const int64_t gi0 = (int64_t)I * tile + r0, gj0 = (int64_t)J * tile + c0;
+    const int nrow = min(kAsmBlk, tile - r0), ncol = min(kAsmBlk, tile - c0);
+
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+
+    double* sA = sm;                       // [dchunk][64]  (d-major so that rows are bank-spread)
+    double* sB = sm + kAsmMaxD * kAsmBlk;  // [dchunk][64]
+    for (int d0 = 0; d0 < D; d0 += kAsmMaxD) {
+        const int dc = min(kAsmMaxD, D - d0);
+        __syncthreads();
+        for (int idx = tid; idx < kAsmBlk * dc; idx += 256) {
+            const int r = idx / dc, d = idx % dc;
+            sA[d * kAsmBlk + r] = (r < nrow) ? A[(gi0 + r) * D + d0 + d] : 0.0;
+            sB[d * kAsmBlk + r] = (r < ncol) ? B[(gj0 + r) * D + d0 + d] : 0.0;
+        }
+        __syncthreads();
+        for (int d = 0; d < dc; ++d) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = sA[d * kAsmBlk + ty + 16 * i];
+            const double2 b01 = *reinterpret_cast<const double2*>(sB + d * kAsmBlk + 4 * tx);
+            const double2 b23 = *reinterpret_cast<const double2*>(sB + d * kAsmBlk + 4 * tx + 2);
+            b[0] = b01.x; b[1] = b01.y; b[2] = b23.x; b[3] = b23.y;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const double diff = a[i] - b[j];
+                    acc[i][j] = fma(diff, diff, acc[i][j]);
+                }
+        }
+    }
+    double* tbase = out + (size_t)tidx * tile * tile;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int r = ty + 16 * i;
+        if (r >= nrow || 4 * tx >= ncol) continue;
+        double k[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            k[j] = se_kernel(acc[i][j], h);
+            if (sym_lower && (gi0 + r) == (gj0 + 4 * tx + j)) k[j] += h.noise;
+        }
+        double* dst = tbase + (size_t)(r0 + r) * tile + c0 + 4 * tx;
+        __stcs(reinterpret_cast<double2*>(dst), make_double2(k[0], k[1]));
+        __stcs(reinterpret_cast<double2*>(dst) + 1, make_double2(k[2], k[3]));
+    }
+}
+
+// tiles -> dense (inspection helper)
+__global__ void tiles_to_dense_kernel(const double* __restrict__ tiles, int64_t n, int64_t nb, int tile, int lower_packed,
+                                      double* __restrict__ dense) {
+    const int64_t total = n * nb;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = idx / nb, j = idx % nb;
+        const int64_t I = i / tile, J = j / tile;
+        double v = 0.0;
+        if (lower_packed) {
+            if (j <= i) v = tiles[((size_t)I * (I + 1) / 2 + J) * tile * tile + (i % tile) * tile + (j % tile)];
+        } else {
+            v = tiles[((size_t)I * (nb / tile) + J) * tile * tile + (i % tile) * tile + (j % tile)];
+        }
+        dense[idx] = v;
+    }
+}
+
+// Sigma: copy the lower triangle onto the upper one so both are bit-identical (reading A12).
+__global__ void mirror_lower_kernel(double* __restrict__ S, int64_t m) {
+    __shared__ double tile[32][33];
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj > bi) return;
+    const int tx = threadIdx.x, ty = threadIdx.y;   // 32 x 8
+    for (int r = ty; r < 32; r += 8) tile[r][tx] = S[((int64_t)bi * 32 + r) * m + (int64_t)bj * 32 + tx];
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        // element (bj*32 + r, bi*32 + tx) <- (bi*32 + tx, bj*32 + r)
+        const int64_t row = (int64_t)bj * 32 + r, col = (int64_t)bi * 32 + tx;
+        if (col > row) S[row * m + col] = tile[tx][r];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Triangular solves for alpha.  Block rows/columns of 128 (kSB) regardless of the
+// tile size (tile % 32 == 0 is handled by kSB = gcd-style choice made on the host: sb divides
+// tile).  One CTA per block row; rows are handed out by a ticket so that a CTA only ever waits
+// for rows claimed before it.  The off-diagonal part is a streaming GEMV that consumes x_p as
+// soon as block p publishes it; the diagonal block is applied as a GEMV with its inverse.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int ld_acquire_i(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ const double* tile_block_ptr(const double* L, int t, int sbt, int gr, int gc, int sb) {
+    const int I = gr / sbt, J = gc / sbt;
+    return L + ((size_t)I * (I + 1) / 2 + J) * (size_t)t * t + (size_t)(gr % sbt) * sb * t + (size_t)(gc % sbt) * sb;
+}
+
+// Forward: x_i = invD_i (y_i - sum_{p<i} L(i,p) x_p).   SB = block edge (32, 64 or 128).
+template <int SB>
+__global__ void __launch_bounds__(256) forward_solve_kernel(const double* __restrict__ L, int t, int NB,
+                                                            const double* __restrict__ invD, const double* __restrict__ y,
+                                                            double* __restrict__ x, int* __restrict__ flags,
+                                                            unsigned int* __restrict__ ticket) {
+    constexpr int TX = SB / 4;            // threads across a row (4 columns each)
+    constexpr int TY = 256 / TX;          // row groups
+    constexpr int RPT = SB / TY;          // rows per thread
+    __shared__ double s_red[SB * (TX + 1)];
+    __shared__ double s_rhs[SB];
+    __shared__ unsigned int s_row;
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+    const int sbt = t / SB;
+    if (tid == 0) s_row = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const int i = (int)s_row;
+    if (i >= NB) return;
+    double acc[RPT];
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) acc[r] = 0.0;
+    for (int pb = 0; pb < i; ++pb) {
+        if (tid == 0) { while (ld_acquire_i(flags + pb) == 0) __nanosleep(32); }
+        __syncthreads();
+        const double* blk = tile_block_ptr(L, t, sbt, i, pb, SB);
+        const double2 x01 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx));
+        const double2 x23 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx + 2));
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const double* row = blk + (size_t)(ty + TY * r) * t + 4 * tx;
+            const double2 l01 = __ldcs(reinterpret_cast<const double2*>(row));
+            const double2 l23 = __ldcs(reinterpret_cast<const double2*>(row) + 1);
+            acc[r] = fma(l01.x, x01.x, acc[r]);
+            acc[r] = fma(l01.y, x01.y, acc[r]);
+            acc[r] = fma(l23.x, x23.x, acc[r]);
+            acc[r] = fma(l23.y, x23.y, acc[r]);
+        }
+    }
+    // reduce the TX partial sums of every row
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) s_red[(ty + TY * r) * (TX + 1) + tx] = acc[r];
+    __syncthreads();
+    if (tid < SB) {
+        double s = 0.0;
+        for (int k = 0; k < TX; ++k) s += s_red[tid * (TX + 1) + k];
+        s_rhs[tid] = y[(size_t)i * SB + tid] - s;
+    }
+    __syncthreads();
+    // x_i = invD_i * rhs  (lower triangular inverse, row-major SB x SB)
+    const double* inv = invD + (size_t)i * SB * SB;
+    double part[RPT];
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) {
+        const double* row = inv + (size_t)(ty + TY * r) * SB + 4 * tx;
+        const double2 l01 = *reinterpret_cast<const double2*>(row);
+        const double2 l23 = *(reinterpret_cast<const double2*>(row) + 1);
+        part[r] = l01.x * s_rhs[4 * tx] + l01.y * s_rhs[4 * tx + 1] + l23.x * s_rhs[4 * tx + 2] + l23.y * s_rhs[4 * tx + 3];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) s_red[(ty + TY * r) * (TX + 1) + tx] = part[r];
+    __syncthreads();
+    if (tid < SB) {
+        double s = 0.0;
+        for (int k = 0; k < TX; ++k) s += s_red[tid * (TX + 1) + k];
+        x[(size_t)i * SB + tid] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) { __threadfence(); atomicExch(flags + i, 1); }
+}
+
+// Backward: x_j = invD_j^T (b_j - sum_{i>j} L(i,j)^T x_i); block columns handed out from the last.
+template <int SB>
+__global__ void __launch_bounds__(256) backward_solve_kernel(const double* __restrict__ L, int t, int NB,
+                                                             const double* __restrict__ invD, const double* __restrict__ b,
+                                                             double* __restrict__ x, int* __restrict__ flags,
+                                                             unsigned int* __restrict__ ticket) {
+    constexpr int TX = SB / 4;
+    constexpr int TY = 256 / TX;
+    constexpr int RPT = SB / TY;
+    __shared__ double s_red[TY * SB];
+    __shared__ double s_rhs[SB];
+    __shared__ unsigned int s_col;
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+    const int sbt = t / SB;
+    if (tid == 0) s_col = atomicAdd(ticket, 1u);
+    __syncthreads();
+    if ((int)s_col >= NB) return;
+    const int j = NB - 1 - (int)s_col;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};     // columns 4tx..4tx+3, partial over this thread's rows
+    for (int ib = NB - 1; ib > j; --ib) {
+        if (tid == 0) { while (ld_acquire_i(flags + ib) == 0) __nanosleep(32); }
+        __syncthreads();
+        const double* blk = tile_block_ptr(L, t, sbt, ib, j, SB);
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const int rr = ty + TY * r;
+            const double xv = __ldcg(x + (size_t)ib * SB + rr);
+            const double* row = blk + (size_t)rr * t + 4 * tx;
+            const double2 l01 = __ldcs(reinterpret_cast<const double2*>(row));
+            const double2 l23 = __ldcs(reinterpret_cast<const double2*>(row) + 1);
+            acc[0] = fma(l01.x, xv, acc[0]);
+            acc[1] = fma(l01.y, xv, acc[1]);
+            acc[2] = fma(l23.x, xv, acc[2]);
+            acc[3] = fma(l23.y, xv, acc[3]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) s_red[ty * SB + 4 * tx + c] = acc[c];
+    __syncthreads();
+    if (tid < SB) {
+        double s = 0.0;
+        for (int k = 0; k < TY; ++k) s += s_red[k * SB + tid];
+        s_rhs[tid] = b[(size_t)j * SB + tid] - s;
+    }
+    __syncthreads();
+    // x_j = invD_j^T rhs:  x[c] = sum_r inv[r][c] rhs[r]
+    const double* inv = invD + (size_t)j * SB * SB;
+    double part[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) {
+        const int rr = ty + TY * r;
+        const double rv = s_rhs[rr];
+        const double* row = inv + (size_t)rr * SB + 4 * tx;
+        const double2 l01 = *reinterpret_cast<const double2*>(row);
+        const double2 l23 = *(reinterpret_cast<const double2*>(row) + 1);
+        part[0] = fma(l01.x, rv, part[0]);
+        part[1] = fma(l01.y, rv, part[1]);
+        part[2] = fma(l23.x, rv, part[2]);
+        part[3] = fma(l23.y, rv, part[3]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 4; ++c) s_red[ty * SB + 4 * tx + c] = part[c];
+    __syncthreads();
+    if (tid < SB) {
+        double s = 0.0;
+        for (int k = 0; k < TY; ++k) s += s_red[k * SB + tid];
+        x[(size_t)j * SB + tid] = s;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) { __threadfence(); atomicExch(flags + j, 1); }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Predictive mean, fused with the cross-covariance: mean[a] = sum_i k(xs_a, x_i) alpha_i.
+// One CTA per kMeanTM test points; each thread strides over training points.  D <= kMeanMaxD staged
+// in registers per training point; the test points live in shared memory.
+// ---------------------------------------------------------------------------------------------
+constexpr int kMeanTM = 8;
+
+__global__ void __launch_bounds__(256) predict_mean_kernel(const double* __restrict__ X, int64_t n, int D,
+                                                           const double* __restrict__ alpha, const double* __restrict__ Xs,
+                                                           int64_t m, HyperDev h, double* __restrict__ mean) {
+    extern __shared__ __align__(16) double sm[];   // [kMeanTM][D] test points, then [kMeanTM][256] reduction
+    double* sXs = sm;
+    double* sRed = sm + kMeanTM * D;
+    const int tid = threadIdx.x;
+    const int64_t a0 = (int64_t)blockIdx.x * kMeanTM;
+    const int na = (int)min((int64_t)kMeanTM, m - a0);
+    for (int idx = tid; idx < kMeanTM * D; idx += 256) {
+        const int a = idx / D, d = idx % D;
+        sXs[idx] = (a < na) ? Xs[(a0 + a) * D + d] : 0.0;
+    }
+    __syncthreads();
+    double acc[kMeanTM];
+#pragma unroll
+    for (int a = 0; a < kMeanTM; ++a) acc[a] = 0.0;
+    for (int64_t i = tid; i < n; i += 256) {
+        double r2[kMeanTM];
+#pragma unroll
+        for (int a = 0; a < kMeanTM; ++a) r2[a] = 0.0;
+        const double* xi = X + i * D;
+        for (int d = 0; d < D; ++d) {
+            const double xv = xi[d];
+#pragma unroll
+            for (int a = 0; a < kMeanTM; ++a) {
+                const double diff = sXs[a * D + d] - xv;
+                r2[a] = fma(diff, diff, r2[a]);
+            }
+        }
+        const double al = alpha[i];
+#pragma unroll
+        for (int a = 0; a < kMeanTM; ++a) acc[a] = fma(se_kernel(r2[a], h), al, acc[a]);
+    }
+#pragma unroll
+    for (int a = 0; a < kMeanTM; ++a) sRed[a * 256 + tid] = acc[a];
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (tid < s) {
+#pragma unroll
+            for (int a = 0; a < kMeanTM; ++a) sRed[a * 256 + tid] += sRed[a * 256 + tid + s];
+        }
+        __syncthreads();
+    }
+    if (tid < na) mean[a0 + tid] = sRed[tid * 256];
+}
+
+}  // namespace gpb

@@ -1,0 +1,291 @@
+#include "gp_schedule.h"
+
+#include <algorithm>
+#include <cstdio>
+#include <functional>
+#include <queue>
+
+namespace gpb {
+namespace {
+
+struct Shape {
+    int M, Mm, nbt, NB, NBm;
+    bool predict;
+    // block id spaces: L [0, NB*NB), V [offV, offV + NBm*NB), S [offS, ...)
+    int64_t offV, offS, nblocks;
+    Shape(int M_, int Mm_, int nbt_, bool predict_) : M(M_), Mm(Mm_), nbt(nbt_), predict(predict_) {
+        NB = M * nbt;
+        NBm = Mm * nbt;
+        offV = (int64_t)NB * NB;
+        offS = offV + (int64_t)NBm * NB;
+        nblocks = offS + (int64_t)NBm * NBm;
+    }
+    int64_t idL(int gr, int gc) const { return (int64_t)gr * NB + gc; }
+    int64_t idV(int gr, int gc) const { return offV + (int64_t)gr * NB + gc; }
+    int64_t idS(int gr, int gc) const { return offS + (int64_t)gr * NBm + gc; }
+    int finL(int gr, int gc) const {
+        const int K = gc / nbt, bk = gc % nbt;
+        return (gr / nbt == K) ? K + 1 + bk : K + 1 + (bk > 0 ? 1 : 0);
+    }
+    int finV(int gc) const { return gc / nbt + 1 + (gc % nbt > 0 ? 1 : 0); }
+};
+
+// The waits and writes of an item, mirroring gp_exec.cuh exactly.
+template <class FW, class FR>
+void item_effects(const Shape& s, const SchedItem& it, FW&& wait, FR&& write) {
+    const int gr = (int)it.gr, gc = (int)it.gc, q0 = (int)(it.q & 0xffffu), q1 = (int)(it.q >> 16);
+    const int nbt = s.nbt;
+    switch (it.op) {
+        case S_UPD_L:
+            wait(s.idL(gr, gc), q0 / nbt + q0 % nbt);
+            for (int q = q0; q < q1; ++q) { wait(s.idL(gr, q), s.finL(gr, q)); wait(s.idL(gc, q), s.finL(gc, q)); }
+            write(s.idL(gr, gc));
+            break;
+        case S_TRSM_L:
+            wait(s.idL(gr, gc), s.finL(gr, gc) - 1);
+            wait(s.idL(gc, gc), s.finL(gc, gc));
+            write(s.idL(gr, gc));
+            break;
+        case S_POTRF:
+            wait(s.idL(gc, gc), s.finL(gc, gc) - 1);
+            write(s.idL(gc, gc));
+            break;
+        case S_ROW_L:
+            for (int jj = 0; jj < nbt; ++jj) {
+                wait(s.idL(gr, gc + jj), gc / nbt);
+                wait(s.idL(gc + jj, gc + jj), s.finL(gc + jj, gc + jj));
+            }
+            for (int jj = 0; jj < nbt; ++jj) {
+                if (jj > 0) write(s.idL(gr, gc + jj));
+                write(s.idL(gr, gc + jj));
+            }
+            break;
+        case S_UPD_V:
+            wait(s.idV(gr, gc), q0 / nbt);
+            for (int q = q0; q < q1; ++q) wait(s.idV(gr, q), s.finV(q));
+            write(s.idV(gr, gc));
+            break;
+        case S_ROW_V:
+            for (int jj = 0; jj < nbt; ++jj) wait(s.idV(gr, gc + jj), gc / nbt);
+            for (int jj = 0; jj < nbt; ++jj) {
+                if (jj > 0) write(s.idV(gr, gc + jj));
+                write(s.idV(gr, gc + jj));
+            }
+            break;
+        case S_UPD_S:
+            wait(s.idS(gr, gc), q0 / nbt);
+            for (int q = q0; q < q1; ++q) { wait(s.idV(gr, q), s.finV(q)); wait(s.idV(gc, q), s.finV(q)); }
+            write(s.idS(gr, gc));
+            break;
+        default: break;
+    }
+}
+
+// cost model in microseconds (B200, FP64 DMMA path; only the ratios matter)
+struct Cost {
+    double per_q, fixed, potrf;
+    explicit Cost(int blk) {
+        if (blk >= 128) { per_q = 19.5; fixed = 4.0; potrf = 45.0; }
+        else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 14.0; }
+        else { per_q = 0.8; fixed = 2.5; potrf = 6.0; }
+    }
+    double of(const SchedItem& it, int nbt) const {
+        const int q0 = (int)(it.q & 0xffffu), q1 = (int)(it.q >> 16);
+        switch (it.op) {
+            case S_UPD_L: case S_UPD_V: case S_UPD_S: return fixed + per_q * (q1 - q0);
+            case S_TRSM_L: return fixed + per_q;
+            case S_POTRF: return potrf;
+            case S_ROW_L: case S_ROW_V: {
+                double c = 0.0;
+                for (int jj = 0; jj < nbt; ++jj) c += (jj > 0 ? fixed + per_q * jj : 0.0) + fixed + per_q;
+                return c;
+            }
+            default: return 1.0;
+        }
+    }
+};
+
+inline SchedItem mk(uint32_t op, int gr, int gc, int q0 = 0, int q1 = 0) {
+    SchedItem it;
+    it.op = op; it.gr = (uint32_t)gr; it.gc = (uint32_t)gc; it.q = (uint32_t)q0 | ((uint32_t)q1 << 16);
+    return it;
+}
+
+void program_order_cholesky(int M, int nbt, std::vector<SchedItem>& v) {
+    for (int J = 0; J < M; ++J) {
+        const int qt = J * nbt;
+        // POTRF tile task = right-looking block Cholesky of the diagonal tile
+        for (int jj = 0; jj < nbt; ++jj) {
+            v.push_back(mk(S_POTRF, qt + jj, qt + jj));
+            for (int ii = jj + 1; ii < nbt; ++ii) v.push_back(mk(S_TRSM_L, qt + ii, qt + jj));
+            for (int kk = jj + 1; kk < nbt; ++kk)
+                for (int ii = kk; ii < nbt; ++ii) v.push_back(mk(S_UPD_L, qt + ii, qt + kk, qt + jj, qt + jj + 1));
+        }
+        // TRSM tile tasks: one chain per block row
+        for (int I = J + 1; I < M; ++I)
+            for (int bi = 0; bi < nbt; ++bi) v.push_back(mk(S_ROW_L, I * nbt + bi, qt));
+        // SYRK and GEMM tile tasks
+        for (int K = J + 1; K < M; ++K)
+            for (int I = K; I < M; ++I)
+                for (int bk = 0; bk < nbt; ++bk)
+                    for (int bi = (I == K ? bk : 0); bi < nbt; ++bi)
+                        v.push_back(mk(S_UPD_L, I * nbt + bi, K * nbt + bk, qt, qt + nbt));
+    }
+}
+
+void program_order_predict(int M, int Mm, int nbt, std::vector<SchedItem>& v) {
+    for (int J = 0; J < M; ++J) {
+        const int qt = J * nbt;
+        for (int a = 0; a < Mm * nbt; ++a) v.push_back(mk(S_ROW_V, a, qt));                      // V^T_{a,J} = (..) L_JJ^-T
+        for (int P = J + 1; P < M; ++P)                                                           // V^T_{a,P} -= V^T_{a,J} L_{P,J}^T
+            for (int bk = 0; bk < nbt; ++bk)
+                for (int a = 0; a < Mm * nbt; ++a) v.push_back(mk(S_UPD_V, a, P * nbt + bk, qt, qt + nbt));
+        for (int b = 0; b < Mm * nbt; ++b)                                                        // Sigma_{a,b} -= V^T_{a,J} V^T_{b,J}^T
+            for (int a = b; a < Mm * nbt; ++a) v.push_back(mk(S_UPD_S, a, b, qt, qt + nbt));
+    }
+}
+
+void schedule(const Shape& s, std::vector<SchedItem>& prog, int workers, int blk, std::vector<SchedItem>& out,
+              SchedStats* stats, bool simulate) {
+    const int N = (int)prog.size();
+    if (!simulate || N == 0) { out = prog; return; }
+    const Cost cost(blk);
+    // 1. writers of every block version
+    std::vector<int32_t> wcount(s.nblocks + 1, 0);
+    for (int i = 0; i < N; ++i) item_effects(s, prog[i], [](int64_t, int) {}, [&](int64_t b) { ++wcount[b + 1]; });
+    for (int64_t b = 0; b < s.nblocks; ++b) wcount[b + 1] += wcount[b];
+    std::vector<int32_t> writer(wcount[s.nblocks]);
+    {
+        std::vector<int32_t> fill(wcount.begin(), wcount.end() - 1);
+        for (int i = 0; i < N; ++i) item_effects(s, prog[i], [](int64_t, int) {}, [&](int64_t b) { writer[fill[b]++] = i; });
+    }
+    // 2. dependency lists (CSR), deduplicated
+    std::vector<int64_t> dep_off(N + 1, 0);
+    std::vector<int32_t> deps;
+    deps.reserve((size_t)N * 4);
+    std::vector<int32_t> tmp;
+    for (int i = 0; i < N; ++i) {
+        tmp.clear();
+        item_effects(s, prog[i],
+                     [&](int64_t b, int need) {
+                         if (need > 0) {
+                             const int32_t w = writer[wcount[b] + need - 1];
+                             if (w != i) tmp.push_back(w);
+                         }
+                     },
+                     [](int64_t) {});
+        std::sort(tmp.begin(), tmp.end());
+        tmp.erase(std::unique(tmp.begin(), tmp.end()), tmp.end());
+        deps.insert(deps.end(), tmp.begin(), tmp.end());
+        dep_off[i + 1] = (int64_t)deps.size();
+    }
+    // 3. bottom levels (critical path to the end) in reverse program order
+    std::vector<float> dur(N), bottom(N);
+    double work = 0.0;
+    for (int i = 0; i < N; ++i) { dur[i] = (float)cost.of(prog[i], s.nbt); bottom[i] = dur[i]; work += dur[i]; }
+    for (int i = N - 1; i >= 0; --i)
+        for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) {
+            const int d = deps[e];
+            bottom[d] = std::max(bottom[d], dur[d] + bottom[i]);
+        }
+    // successor CSR
+    std::vector<int64_t> suc_off(N + 1, 0);
+    for (int64_t e = 0; e < (int64_t)deps.size(); ++e) ++suc_off[deps[e] + 1];
+    for (int i = 0; i < N; ++i) suc_off[i + 1] += suc_off[i];
+    std::vector<int32_t> sucs(deps.size());
+    {
+        std::vector<int64_t> fill(suc_off.begin(), suc_off.end() - 1);
+        for (int i = 0; i < N; ++i)
+            for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) sucs[fill[deps[e]]++] = i;
+    }
+    // 4. list scheduling
+    std::vector<int32_t> missing(N);
+    using PR = std::pair<float, int32_t>;                       // (bottom level, -item) max-heap
+    std::priority_queue<PR> ready;
+    for (int i = 0; i < N; ++i) {
+        missing[i] = (int32_t)(dep_off[i + 1] - dep_off[i]);
+        if (missing[i] == 0) ready.push(PR(bottom[i], -i));
+    }
+    using EV = std::pair<double, int32_t>;                      // (finish time, item) min-heap
+    std::priority_queue<EV, std::vector<EV>, std::greater<EV>> running;
+    out.clear();
+    out.reserve(N);
+    int idle = workers;
+    double now = 0.0, makespan = 0.0;
+    while ((int)out.size() < N) {
+        while (idle > 0 && !ready.empty()) {
+            const int i = -ready.top().second;
+            ready.pop();
+            out.push_back(prog[i]);
+            running.push(EV(now + dur[i], i));
+            --idle;
+        }
+        if (running.empty()) break;   // cannot happen for a valid DAG
+        // advance to the next completion (and everything finishing at the same instant)
+        now = running.top().first;
+        while (!running.empty() && running.top().first <= now) {
+            const int i = running.top().second;
+            running.pop();
+            ++idle;
+            for (int64_t e = suc_off[i]; e < suc_off[i + 1]; ++e) {
+                const int sc = sucs[e];
+                if (--missing[sc] == 0) ready.push(PR(bottom[sc], -sc));
+            }
+        }
+        makespan = now;
+    }
+    while (!running.empty()) { makespan = std::max(makespan, running.top().first); running.pop(); }
+    if (stats) {
+        stats->makespan_us = makespan;
+        stats->work_us = work;
+        stats->edges = (int64_t)deps.size();
+        float cp = 0.f;
+        for (int i = 0; i < N; ++i) cp = std::max(cp, bottom[i]);
+        stats->critical_path_us = cp;
+    }
+}
+
+}  // namespace
+
+void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate) {
+    std::vector<SchedItem> prog;
+    program_order_cholesky(M, nbt, prog);
+    schedule(Shape(M, 0, nbt, false), prog, workers, blk, out, stats, simulate);
+}
+
+void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate) {
+    std::vector<SchedItem> prog;
+    program_order_predict(M, Mm, nbt, prog);
+    schedule(Shape(M, Mm, nbt, true), prog, workers, blk, out, stats, simulate);
+}
+
+bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why) {
+    const Shape s(M, predict ? Mm : 0, nbt, predict);
+    std::vector<int32_t> ver(s.nblocks, 0);
+    static const char* kWait = "an item waits for a version no earlier item produces";
+    static const char* kFinal = "a block does not end at its final version";
+    static const char* kCount = "wrong number of items";
+    bool ok = true;
+    for (const SchedItem& it : items) {
+        item_effects(s, it, [&](int64_t b, int need) { if (ver[b] < need) ok = false; }, [&](int64_t b) { ++ver[b]; });
+        if (!ok) { if (why) *why = kWait; return false; }
+    }
+    if (!predict) {
+        for (int gr = 0; gr < s.NB; ++gr)
+            for (int gc = 0; gc <= gr; ++gc)
+                if (ver[s.idL(gr, gc)] != s.finL(gr, gc)) { if (why) *why = kFinal; return false; }
+    } else {
+        for (int gr = 0; gr < s.NBm; ++gr) {
+            for (int gc = 0; gc < s.NB; ++gc)
+                if (ver[s.idV(gr, gc)] != s.finV(gc)) { if (why) *why = kFinal; return false; }
+            for (int gc = 0; gc <= gr; ++gc)
+                if (ver[s.idS(gr, gc)] != M) { if (why) *why = kFinal; return false; }
+        }
+    }
+    std::vector<SchedItem> prog;
+    if (predict) program_order_predict(M, Mm, nbt, prog); else program_order_cholesky(M, nbt, prog);
+    if (prog.size() != items.size()) { if (why) *why = kCount; return false; }
+    return true;
+}
+
+}  // namespace gpb

@@ -1,0 +1,41 @@
+// gp_schedule.h -- host-side construction of the static work-item order the persistent executor
+// (gp_exec.cuh) consumes.  Pure C++ (no CUDA): testable on a machine without a GPU.
+//
+// The tile-task DAG of PAPER.md Fig. 1 (reading A4) is expanded into block-level work items in
+// program order, the dependencies the device enforces with version counters are recovered
+// explicitly, and a list-scheduling simulation on `workers` virtual SMs (critical-path-first
+// priority, per-item cost model) decides the order in which items are handed out.  The order is
+// a topological order of the DAG by construction, which is what makes the in-order ticket
+// scheme deadlock-free; the simulated timing only has to be roughly right for waits to be short.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+namespace gpb {
+
+struct SchedItem {   // must match gpb::Item (gp_exec.cuh)
+    uint32_t op, gr, gc, q;
+};
+
+enum SchedOp : uint32_t {
+    S_UPD_L = 0, S_TRSM_L = 1, S_POTRF = 2, S_ROW_L = 3, S_UPD_V = 4, S_ROW_V = 5, S_UPD_S = 6,
+};
+
+struct SchedStats {
+    double makespan_us = 0.0;       // simulated
+    double work_us = 0.0;           // sum of item costs
+    double critical_path_us = 0.0;
+    int64_t edges = 0;
+};
+
+// M = n / tile, nbt = tile / block, Mm = m / tile.  `blk` (32/64/128) selects the cost model.
+void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>& out, int blk = 128,
+                             SchedStats* stats = nullptr, bool simulate = true);
+void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk = 128,
+                            SchedStats* stats = nullptr, bool simulate = true);
+
+// Checks that `items` is a valid execution order (every wait of every item is satisfied by items
+// earlier in the list) and that every block ends at its final version.  Used by the CPU tests.
+bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why);
+
+}  // namespace gpb

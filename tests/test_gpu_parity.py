@@ -1,0 +1,177 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances are north_star's: relative Frobenius error <= 1e-10 on L,
+<= 1e-9 on mean and Sigma (additionally alpha <= 1e-9, K <= 1e-14; reading A11)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from helpers import relerr
+from paper_2602_19683_b200 import nfir
+
+TOL_K, TOL_L, TOL_ALPHA, TOL_MEAN, TOL_SIGMA = 1e-14, 1e-10, 1e-9, 1e-9, 1e-9
+
+
+@pytest.fixture(scope="module")
+def gp():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    from paper_2602_19683_b200 import binding
+    binding.load()
+    return binding
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _run_pipeline(gp, X, y, Xs, h, tile, width=0):
+    n, D = X.shape
+    m = Xs.shape[0]
+    pipe = gp.GpPipeline(n, m, D, tile, gp.Hyper(h.lengthscale, h.vertical, h.noise, h.ell_squared), sched_width=width)
+    dX, dy, dXs = _dev(X), _dev(y), _dev(Xs)
+    pipe.assemble(dX)
+    K = pipe.dense_L().cpu().numpy()           # lower triangle of K (strict upper zeroed)
+    res = pipe.run(dX, dy, dXs)
+    torch.cuda.synchronize()
+    L = pipe.dense_L().cpu().numpy()
+    return dict(K=K, L=L, alpha=res.alpha.cpu().numpy(), beta=res.beta.cpu().numpy(), mean=res.mean.cpu().numpy(),
+                Sigma=res.Sigma.cpu().numpy(), info=int(res.info.item()))
+
+
+def _check_against_oracle(out, p):
+    assert out["info"] == 0
+    assert relerr(out["K"], np.tril(p.K)) <= TOL_K
+    assert relerr(out["L"], p.L) <= TOL_L
+    assert relerr(out["beta"], p.beta) <= TOL_ALPHA
+    assert relerr(out["alpha"], p.alpha) <= TOL_ALPHA
+    assert relerr(out["mean"], p.mean) <= TOL_MEAN
+    assert relerr(out["Sigma"], p.Sigma) <= TOL_SIGMA
+    assert np.array_equal(out["Sigma"], out["Sigma"].T)          # exactly symmetric (reading A12)
+    # element-wise, so that a misplaced block cannot hide in a norm
+    np.testing.assert_allclose(out["L"], p.L, rtol=0, atol=1e-9 * np.abs(p.L).max())
+    np.testing.assert_allclose(out["Sigma"], p.Sigma, rtol=0, atol=1e-9 * np.abs(p.Sigma).max())
+
+
+@pytest.mark.parametrize("ci", [0, 1])
+def test_configs_full_pipeline(gp, ci):
+    cfg = nfir.CONFIGS[ci]
+    X, y, Xs = nfir.make_inputs(cfg)
+    h = oracle.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    p = oracle.predict(X, y, Xs, h)
+    out = _run_pipeline(gp, X, y, Xs, h, cfg.tile)
+    _check_against_oracle(out, p)
+
+
+@pytest.mark.parametrize("n,m,D,tile", [
+    (96, 32, 3, 32),        # block 32, 3x3 tiles, odd D
+    (192, 64, 5, 64),       # block 64
+    (384, 128, 8, 128),     # block 128, one block per tile
+    (768, 256, 8, 256),     # block 128, 2x2 blocks per tile, 3x3 tiles
+    (1536, 384, 8, 384),    # 3x3 blocks per tile, 4 tiles
+    (640, 128, 16, 128),    # 5 tiles of one block, D=16
+    (1024, 512, 8, 512),    # 4 blocks per tile edge
+    (320, 320, 8, 160),     # tile 160 -> block 32, 5 blocks per tile edge
+])
+def test_shapes_spanning_tiles_and_blocks(gp, n, m, D, tile):
+    X, y = nfir.nfir_features(n + m + D, n, D)
+    Xs, _ = nfir.nfir_features(7 * n + 1, m, D, with_targets=False)
+    h = oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h)
+    out = _run_pipeline(gp, X, y, Xs, h, tile)
+    _check_against_oracle(out, p)
+
+
+def test_config4_hyperparameters_and_ell_switch(gp):
+    X, y = nfir.nfir_features(5, 512, 16)
+    Xs, _ = nfir.nfir_features(6, 256, 16, with_targets=False)
+    for h in (oracle.Hyper(2.0, 1.0, 0.05, False), oracle.Hyper(2.0, 1.0, 0.05, True)):
+        p = oracle.predict(X, y, Xs, h)
+        out = _run_pipeline(gp, X, y, Xs, h, 256)
+        _check_against_oracle(out, p)
+
+
+def test_worked_examples_on_gpu_padded(gp, golden):
+    """The 40-digit examples cannot be tiled (n=2,3); embed them far away from 30/29 filler points so the
+    leading block of L and the predictions of the real test points are unchanged."""
+    g = golden["B"]
+    X3, y3, Xs2 = np.array(g["X"]), np.array(g["y"]), np.array(g["Xs"])
+    n, m = 32, 32
+    X = np.zeros((n, 2)); y = np.zeros(n); Xs = np.zeros((m, 2))
+    X[:3], y[:3], Xs[:2] = X3, y3, Xs2
+    X[3:, 0] = 1000.0 + 100.0 * np.arange(n - 3)      # kernel underflows to exactly 0 against everything
+    Xs[2:, 1] = -1000.0 - 100.0 * np.arange(m - 2)
+    out = _run_pipeline(gp, X, y, Xs, oracle.Hyper(), 32)
+    Lg = np.array([[float(t) for t in r] for r in g["L"]])
+    np.testing.assert_allclose(out["L"][:3, :3], Lg, rtol=1e-13, atol=1e-15)
+    np.testing.assert_allclose(out["alpha"][:3], [float(t) for t in g["alpha"]], rtol=1e-12)
+    np.testing.assert_allclose(out["mean"][:2], [float(t) for t in g["mean"]], rtol=1e-12)
+    Sg = np.array([[float(t) for t in r] for r in g["Sigma"]])
+    np.testing.assert_allclose(out["Sigma"][:2, :2], Sg, rtol=1e-12)
+
+
+def test_tile_size_independence(gp):
+    cfg = nfir.CONFIGS[1]
+    X, y, Xs = nfir.make_inputs(cfg)
+    h = oracle.Hyper()
+    ref = _run_pipeline(gp, X, y, Xs, h, 1024)     # one tile = untiled
+    for tile in (32, 128, 256, 512):
+        out = _run_pipeline(gp, X, y, Xs, h, tile)
+        assert relerr(out["L"], ref["L"]) <= 1e-11
+        assert relerr(out["mean"], ref["mean"]) <= 1e-11
+        assert relerr(out["Sigma"], ref["Sigma"]) <= 1e-11
+
+
+@pytest.mark.parametrize("width", [1, 2, 7, 148])
+def test_scheduler_width_does_not_change_results(gp, width):
+    X, y = nfir.nfir_features(3, 768, 8)
+    Xs, _ = nfir.nfir_features(4, 256, 8, with_targets=False)
+    h = oracle.Hyper()
+    a = _run_pipeline(gp, X, y, Xs, h, 256, width=0)
+    b = _run_pipeline(gp, X, y, Xs, h, 256, width=width)
+    for k in ("L", "alpha", "mean", "Sigma"):
+        assert np.array_equal(a[k], b[k]), k          # same item order per block -> bitwise identical
+
+
+def test_not_positive_definite_reports_column_and_terminates(gp):
+    n, tile = 256, 128
+    K = np.eye(n)
+    K[200, 200] = -1.0
+    tiles = []
+    M = n // tile
+    for I in range(M):
+        for J in range(I + 1):
+            tiles.append(K[I * tile:(I + 1) * tile, J * tile:(J + 1) * tile].ravel())
+    KL = _dev(np.concatenate(tiles))
+    cb, _, _ = gp.gp_workspace_bytes(n, 0, 1, tile)
+    work = torch.empty(cb, dtype=torch.uint8, device="cuda")
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    gp.gp_cholesky_tiled(KL, n, tile, 0, info, work)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 201
+
+
+def test_argument_errors(gp):
+    X = torch.zeros(64, 4, dtype=torch.float64, device="cuda")
+    out = torch.zeros(64 * 64, dtype=torch.float64, device="cuda")
+    h = gp.Hyper()
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_assemble_tiles(X, X, h, 48, gp.GP_SYM_LOWER, out)
+    assert e.value.code == gp.ERR["TILE"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_assemble_tiles(X, X, gp.Hyper(lengthscale=-1.0), 32, gp.GP_SYM_LOWER, out)
+    assert e.value.code == gp.ERR["HYPER"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_assemble_tiles(X, X, h, 32, 5, out)
+    assert e.value.code == gp.ERR["MODE"]
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    small = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_cholesky_tiled(out, 64, 32, 0, info, small)
+    assert e.value.code == gp.ERR["WORKSPACE"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_cholesky_tiled(out, 70, 32, 0, info, small)
+    assert e.value.code == gp.ERR["TILE"]

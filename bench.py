@@ -1,0 +1,419 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of the GP prediction pipeline (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl b200|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+One "step" is one pass of the whole hot path over one batch of
+synthetic NFIR-shaped input: assemble K, tiled Cholesky, both
+triangular solves, predictive mean, full predictive covariance.  Every phase is bracketed by CUDA
+events on the launching stream; `value` is the Cholesky rate n^3/3 / t_cholesky summed over all
+ranks (replicas only: each GPU factors its own problem, no data-path collective, DESIGN.md
+"Multi-GPU").  Rank 0 prints ONE JSON line.
+
+`--impl reference` times the CPU oracle (oracle/, the only reference this tier has) on a bounded
+sample of the same workload on the box's host cores.
+
+Extras (not part of the default line): `--sweep` runs the config-2 tile-size x scheduler-width
+sweep (analogue of the paper's Fig. 3) and `--cusolver-ref` times cuSOLVER potrf
+once through torch.linalg.cholesky as a reported reference; both print JSON lines
+of their own.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "FP64 tiled Cholesky GFLOP/s and full-cov prediction time at n=32768; % FP64 peak"
+
+# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant
+# kernel (exec_kernel<128>, the Cholesky DAG) from the ncu --set full capture summarised in
+# profiles/; keyed by (n, tile).  None = not captured for this workload.
+NCU_TRAFFIC_BYTES = {}
+
+ORACLE_SAMPLE_BASELINE = (4096, 512)    # (n, m) of the cpu_baseline leg: ~10-30 s of CPU work
+ORACLE_SAMPLE_REFERENCE = (3072, 384)   # per step of --impl reference
+
+
+def _parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (default 3: the headline)")
+    ap.add_argument("--tile", type=int, default=0, help="override the config's tile size")
+    ap.add_argument("--width", type=int, default=0, help="scheduler width (persistent CTAs), 0 = one per SM")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--cusolver-ref", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, f"/tmp/gp_b200_clocks_{os.getpid()}.csv"
+
+    def start(self):
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.f.close()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        with open(self.path) as f:
+            for line in f:
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 7:
+                    continue
+                try:
+                    sm.append(float(p[0])); smax.append(float(p[1])); power.append(float(p[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, p[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        try:
+            os.remove(self.path)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # samples under load = upper half (the sampler also sees the idle edges of the region)
+        load = sorted(sm)[len(sm) // 2:]
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(smax), "power_w_max": max(power),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    return rank, local, world
+
+
+def _config(args):
+    from paper_2602_19683_b200 import nfir
+    cfg = nfir.CONFIGS[args.config]
+    tile = args.tile or cfg.tile
+    return cfg, tile
+
+
+def _config_dict(cfg, tile, width, world):
+    M = cfg.n // tile
+    return {"workload": f"c{cfg.index}: n={cfg.n} m={cfg.m} D={cfg.D} tile={tile} ({M}x{M} tiles) FP64, NFIR-shaped synthetic",
+            "n": cfg.n, "m": cfg.m, "D": cfg.D, "tile": tile, "sched_width": width or "auto (one CTA per SM)",
+            "lengthscale": cfg.lengthscale, "vertical": cfg.vertical, "noise": cfg.noise,
+            "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+            "l2": "inputs larger than L2 (K tiles %.2f GB re-assembled every step)" % (M * (M + 1) / 2 * tile * tile * 8 / 1e9)}
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_run(n, m, D, cfg, seed_shift=0):
+    """One oracle pass (a1-a12) on an (n, m) sample of the workload; returns per-phase seconds."""
+    import oracle
+    from paper_2602_19683_b200 import nfir
+    X, y = nfir.nfir_features(1000 + cfg.index + seed_shift, n, D)
+    Xs, _ = nfir.nfir_features(2000 + cfg.index + seed_shift, m, D, with_targets=False)
+    h = oracle.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    t0 = time.perf_counter()
+    K = oracle.assemble(X, X, h, True)
+    t1 = time.perf_counter()
+    L = oracle.cholesky(K)
+    t2 = time.perf_counter()
+    beta = oracle.forward_subst(L, y)
+    alpha = oracle.backward_subst(L, beta)
+    fitted = oracle.Prediction(K=None, L=L, beta=beta, alpha=alpha)
+    oracle.predict(X, y, Xs, h, full_cov=True, fitted=fitted)
+    t3 = time.perf_counter()
+    return {"assemble_s": t1 - t0, "cholesky_s": t2 - t1, "predict_s": t3 - t2, "total_s": t3 - t0}
+
+
+def cpu_baseline(cfg):
+    import oracle
+    n, m = ORACLE_SAMPLE_BASELINE
+    n, m = min(n, cfg.n), min(m, cfg.m)
+    r = oracle_run(n, m, cfg.D, cfg)
+    return {"value": n ** 3 / 3.0 / r["cholesky_s"] / 1e9, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"one oracle pass on n={n}, m={m}, D={cfg.D} of the same generator (unblocked Cholesky {r['cholesky_s']:.2f} s, "
+                      f"whole pipeline {r['total_s']:.2f} s)",
+            "predict_full_cov_ms": r["predict_s"] * 1e3, "cholesky_ms": r["cholesky_s"] * 1e3}
+
+
+def run_reference(args):
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    cfg, tile = _config(args)
+    n, m = ORACLE_SAMPLE_REFERENCE
+    n, m = min(n, cfg.n), min(m, cfg.m)
+    for _ in range(args.warmup):
+        oracle_run(n, m, cfg.D, cfg)
+    chol, total, pred = 0.0, 0.0, 0.0
+    for s in range(args.steps):
+        r = oracle_run(n, m, cfg.D, cfg)
+        chol += r["cholesky_s"]; total += r["total_s"]; pred += r["predict_s"]
+    value = args.steps * (n ** 3 / 3.0) / chol / 1e9
+    sample = f"each step = one oracle pass on n={n}, m={m}, D={cfg.D} of the same generator"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": _config_dict(cfg, tile, args.width, world),
+            "predict_full_cov_ms": pred / args.steps * 1e3, "gpu_launches": 0,
+            "cpu_baseline": {"value": value, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+def measure_fp64_peak(gp, torch):
+    """DMMA / DFMA register-resident microbenchmarks: burst (best of 10 short launches) and
+    sustained (back to back for ~2 s), in TFLOP/s."""
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    out = {}
+    for mode, name in ((0, "dmma"), (1, "dfma")):
+        iters = 20000 if mode == 0 else 40000
+        for _ in range(3):
+            flops = gp.gp_fp64_peak_launch(mode, iters, sink)
+        torch.cuda.synchronize()
+        best = 0.0
+        for _ in range(10):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); gp.gp_fp64_peak_launch(mode, iters, sink); b.record(); torch.cuda.synchronize()
+            best = max(best, flops / (a.elapsed_time(b) * 1e-3) / 1e12)
+        out[name + "_burst_tflops"] = best
+        if mode == 0:
+            one = flops / (best * 1e12)
+            reps = max(4, int(2.0 / one))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(reps):
+                gp.gp_fp64_peak_launch(mode, iters, sink)
+            b.record(); torch.cuda.synchronize()
+            out["dmma_sustained_tflops"] = reps * flops / (a.elapsed_time(b) * 1e-3) / 1e12
+    return out
+
+
+LAUNCHES_PER_STEP = {"assemble": 1, "cholesky": 1, "solve": 3, "mean": 1, "full_cov": 5}   # kernels of libgp_b200.so
+
+
+def run_b200(args):
+    import torch
+    rank, local, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl b200 needs a CUDA device: there is no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2602_19683_b200 import binding as gp, nfir
+    gp.load()
+    cfg, tile = _config(args)
+    n, m, D = cfg.n, cfg.m, cfg.D
+    h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    # every replica gets its own seeded problem of the same shape
+    X, y = nfir.nfir_features(1000 + cfg.index + 10 * rank, n, D)
+    Xs, _ = nfir.nfir_features(2000 + cfg.index + 10 * rank, m, D, with_targets=False)
+    hX, hY, hXs = (torch.from_numpy(a).pin_memory() for a in (X, y, Xs))
+    dX, dY, dXs = hX.cuda(), hY.cuda(), hXs.cuda()
+    pipe = gp.GpPipeline(n, m, D, tile, h, sched_width=args.width)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    names = ("assemble", "cholesky", "solve", "mean", "full_cov")
+
+    def step(ev=None):
+        def mark(i):
+            if ev is not None:
+                ev[i].record()
+        mark(0); pipe.assemble(dX)
+        mark(1); pipe.cholesky()
+        mark(2); pipe.solve(dY)
+        mark(3); gp.gp_predict_mean(dX, pipe.alpha, dXs, h, pipe.mean)
+        mark(4); gp.gp_predict_full_cov(pipe.KL, dX, dXs, h, tile, args.width, pipe.Sigma, pipe.work)
+        mark(5)
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    for s in range(args.steps):
+        step(events[s])
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    info = int(pipe.info.item())
+    phase = {nm: sum(events[s][i].elapsed_time(events[s][i + 1]) for s in range(args.steps)) for i, nm in enumerate(names)}
+    total_ms = sum(events[s][0].elapsed_time(events[s][5]) for s in range(args.steps))
+    per_step_chol = [events[s][1].elapsed_time(events[s][2]) for s in range(args.steps)]
+
+    # end to end through the host-buffer C-ABI call: H2D of X, y, X^ and D2H of mean, Sigma inside
+    ws = torch.empty(gp.gp_pipeline_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
+    hMean = torch.empty(m, dtype=torch.float64).pin_memory()
+    hSigma = torch.empty(m, m, dtype=torch.float64).pin_memory()
+    del pipe
+    for _ in range(min(args.warmup, 2)):
+        gp.gp_pipeline_host(hX, hY, hXs, h, tile, args.width, hMean, hSigma, None, ws)
+    barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(args.steps):
+        info_e2e = gp.gp_pipeline_host(hX, hY, hXs, h, tile, args.width, hMean, hSigma, None, ws)
+    b.record()
+    barrier()
+    e2e_ms = a.elapsed_time(b)
+    del ws
+
+    t = torch.tensor([phase[nm] for nm in names] + [total_ms, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    t = t.tolist()
+    phase = {nm: t[i] / args.steps for i, nm in enumerate(names)}
+    total_ms, e2e_ms = t[5] / args.steps, t[6] / args.steps
+
+    if rank == 0:
+        flop = n ** 3 / 3.0
+        chol_gflops = world * flop / (phase["cholesky"] * 1e-3) / 1e9
+        peaks = measure_fp64_peak(gp, torch)
+        peak = peaks["dmma_sustained_tflops"]
+        achieved = flop / (phase["cholesky"] * 1e-3) / 1e12
+        traffic = NCU_TRAFFIC_BYTES.get((n, tile))
+        try:
+            mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            mp = {}
+        line = {
+            "metric": METRIC, "value": chol_gflops, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": _config_dict(cfg, tile, args.width, world),
+            "cholesky_ms": phase["cholesky"], "cholesky_ms_per_step": per_step_chol,
+            "predict_full_cov_ms": phase["solve"] + phase["mean"] + phase["full_cov"],
+            "phases_ms": phase, "info": info,
+            "pct_fp64_peak": 100.0 * achieved / peak,
+            "e2e": {"value": world * flop / (e2e_ms * 1e-3) / 1e9, "unit": "GFLOP/s (n^3/3 over the whole host-to-host pipeline time)",
+                    "ms": e2e_ms, "h2d_bytes_per_step": (n * D + n + m * D) * 8, "d2h_bytes_per_step": (m + m * m) * 8 + 4,
+                    "info": info_e2e, "call": "gp_pipeline_host (pinned host buffers)"},
+            "gpu_launches": sum(LAUNCHES_PER_STEP.values()) * args.steps,
+            "roofline": {"bound": "tensor", "kernel": "exec_kernel<128> (tiled Cholesky DAG: POTRF/TRSM/SYRK/GEMM, FP64 DMMA)",
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                         "peak_source": "gp_fp64_peak_launch DMMA.8x8x4 register-resident microbenchmark, measured live, "
+                                        "sustained ~2 s loop (kernel is timed inside a long step)",
+                         "peak_burst": peaks["dmma_burst_tflops"], "dfma_burst": peaks["dfma_burst_tflops"],
+                         "frac_of_burst": achieved / peaks["dmma_burst_tflops"],
+                         "hbm_gbs_measured": mp.get("hbm_gbs"),
+                         "assemble_gbs": (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["assemble"] * 1e-3) / 1e9,
+                         "solve_gbs": 2 * (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["solve"] * 1e-3) / 1e9},
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(cfg)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+def run_sweep(args):
+    """Config 2: tile in {256,512,1024} x scheduler width in {1,2,4,8,auto}; Cholesky + full-cov."""
+    import torch
+    from paper_2602_19683_b200 import binding as gp, nfir
+    cfg = nfir.CONFIGS[2]
+    n, m, D = cfg.n, cfg.m, cfg.D
+    X, y, Xs = nfir.make_inputs(cfg)
+    dX, dY, dXs = (torch.from_numpy(a).cuda() for a in (X, y, Xs))
+    h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    rows = []
+    for tile in (256, 512, 1024):
+        for width in (1, 2, 4, 8, 0):
+            pipe = gp.GpPipeline(n, m, D, tile, h, sched_width=width)
+            reps = 2 if width in (1, 2) else 5
+            tc, tp = [], []
+            for r in range(reps + 1):
+                pipe.assemble(dX)
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                e[0].record(); pipe.cholesky(); e[1].record()
+                pipe.solve(dY); pipe.predict(dX, dXs, True); e[2].record()
+                torch.cuda.synchronize()
+                if r > 0:
+                    tc.append(e[0].elapsed_time(e[1])); tp.append(e[1].elapsed_time(e[2]))
+            rows.append({"tile": tile, "sched_width": width or "auto", "cholesky_ms": statistics.mean(tc),
+                         "cholesky_gflops": n ** 3 / 3.0 / (statistics.mean(tc) * 1e-3) / 1e9, "predict_full_cov_ms": statistics.mean(tp)})
+            del pipe
+    print(json.dumps({"sweep": "c2 n=8192 m=1024 D=8: tile x scheduler width (PAPER.md:169 analogue)", "rows": rows}), flush=True)
+    return 0
+
+
+def run_cusolver_ref(args):
+    """cuSOLVER potrf on the dense matrix, once, as a reported reference only."""
+    import torch
+    from paper_2602_19683_b200 import binding as gp, nfir
+    cfg, tile = _config(args)
+    n = cfg.n
+    X, _ = nfir.nfir_features(1000 + cfg.index, n, cfg.D)
+    dX = torch.from_numpy(X).cuda()
+    h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    K = torch.empty(n * n, dtype=torch.float64, device="cuda")
+    gp.gp_assemble_tiles(dX, dX, h, n, gp.GP_GENERAL, K)      # one tile of edge n = the dense matrix
+    K = K.view(n, n)
+    K.diagonal().add_(cfg.noise)
+    torch.linalg.cholesky(K[:1024, :1024].clone())            # library warm-up
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); L = torch.linalg.cholesky(K); b.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    print(json.dumps({"reference_only": "cuSOLVER potrf via torch.linalg.cholesky (out of place, dense)", "n": n, "ms": ms,
+                      "gflops": n ** 3 / 3.0 / (ms * 1e-3) / 1e9}), flush=True)
+    return 0
+
+
+def main():
+    args = _parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    if args.cusolver_ref:
+        return run_cusolver_ref(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -125,6 +125,36 @@ int gp_tiles_to_dense(const double* dTiles, int64_t n, int64_t nb, int tile, int
  * runs for an n x n factorisation with this tile size (a6 bookkeeping; host only). */
 int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* work_items);
 
+/* Whole pipeline with HOST buffers -- PAPER.md:143 ("explicit H2D of X, y, X^; only results are
+ * copied back"): the call a user with data in host memory makes.  Copies hX [n x D], hY [n] and
+ * hXs [m x D] to the device, runs a1-a12 (gp_assemble_tiles, gp_cholesky_tiled, gp_solve,
+ * gp_predict_mean, gp_predict_full_cov) on `stream`, copies the results back and SYNCHRONISES the
+ * stream before returning (the only entry point that does; its outputs are host memory).
+ *   hMean [m], hSigma [m x m] (may be NULL: mean only), hAlpha [n] (may be NULL): host outputs;
+ *   pinned host memory makes the copies asynchronous DMA, pageable memory also works.
+ *   h_info: host int, as d_info of gp_cholesky_tiled.
+ *   dWork/work_bytes: DEVICE scratch of at least gp_pipeline_workspace_bytes(); holds X, y, X^,
+ *        the K/L tiles, alpha, beta, mean, Sigma and the per-call scratch. */
+int gp_pipeline_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* bytes);
+int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D,
+                     gp_hyper h, int tile, int sched_width, double* hMean, double* hSigma, double* hAlpha,
+                     int* h_info, void* dWork, size_t work_bytes, void* stream);
+
+/* FP64 peak microbenchmark launch (measurement support; north_star: "FP64 peak also measured by a
+ * microbenchmark").  Enqueues one launch of independent register-resident chains on every SM:
+ * mode 0 = DMMA.8x8x4 (mma.sync.m8n8k4.f64), mode 1 = DFMA.  *flops (host, may be NULL) receives
+ * the floating-point operations one launch performs; the caller times the launch with events.
+ *   d_sink: device double[1], never actually written. */
+int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void* stream);
+
+/* Host-only self-check of the static work-item schedule the persistent executor consumes (a6):
+ * builds the schedule for (n, m, tile) with `workers` virtual SMs (m == 0: Cholesky schedule,
+ * m > 0: predictor schedule) and replays it against the dependency rules of the device code.
+ * Returns GP_OK if every wait of every item is satisfied by earlier items and every block ends at
+ * its final version, GP_ERR_SIZE otherwise.  stats (may be NULL) receives
+ * {items, dependency edges, simulated makespan us, total work us, critical path us}. */
+int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5);
+
 /* Drop the cached device-resident schedules (synchronises the device). */
 void gp_release_cached_schedules(void);
 

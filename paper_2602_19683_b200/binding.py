@@ -21,7 +21,7 @@ ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA":
 
 EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
-           "gp_block_size", "gp_strerror")
+           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck")
 
 
 class gp_hyper(ctypes.Structure):
@@ -72,6 +72,10 @@ def load() -> ctypes.CDLL:
     lib.gp_release_cached_schedules.restype = None
     lib.gp_block_size.argtypes = [ci]
     lib.gp_strerror.argtypes = [ci]
+    lib.gp_pipeline_workspace_bytes.argtypes = [i64, i64, ci, ci, psz]
+    lib.gp_pipeline_host.argtypes = [vp, vp, vp, i64, i64, ci, gp_hyper, ci, ci, vp, vp, vp, vp, vp, sz, vp]
+    lib.gp_schedule_selfcheck.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.gp_fp64_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.gp_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
         if name not in ("gp_release_cached_schedules", "gp_strerror"):
@@ -159,6 +163,46 @@ def gp_predict_full_cov(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: H
 def gp_tiles_to_dense(tiles: torch.Tensor, n: int, nb: int, tile: int, lower_packed: bool, dense: torch.Tensor) -> torch.Tensor:
     _check(load().gp_tiles_to_dense(_ptr(tiles), n, nb, tile, int(lower_packed), _ptr(dense), _stream()), "gp_tiles_to_dense")
     return dense
+
+
+def gp_pipeline_workspace_bytes(n: int, m: int, D: int, tile: int) -> int:
+    b = ctypes.c_size_t(0)
+    _check(load().gp_pipeline_workspace_bytes(n, m, D, tile, ctypes.byref(b)), "gp_pipeline_workspace_bytes")
+    return int(b.value)
+
+
+def _hptr(t: torch.Tensor | None, dtype=torch.float64):
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"expected a contiguous host {dtype} tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def gp_pipeline_host(hX: torch.Tensor, hY: torch.Tensor, hXs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
+                     hMean: torch.Tensor, hSigma: torch.Tensor | None, hAlpha: torch.Tensor | None, work: torch.Tensor) -> int:
+    """HOST tensors in, HOST tensors out (pinned recommended); `work` is device scratch. Returns info."""
+    n, D = hX.shape
+    m = hXs.shape[0]
+    info = ctypes.c_int(0)
+    _check(load().gp_pipeline_host(_hptr(hX), _hptr(hY), _hptr(hXs), n, m, D, h.c(), tile, sched_width, _hptr(hMean),
+                                   _hptr(hSigma), _hptr(hAlpha), ctypes.byref(info), _ptr(work, torch.uint8), work.numel(),
+                                   _stream()), "gp_pipeline_host")
+    return int(info.value)
+
+
+def gp_fp64_peak_launch(mode: int, iters: int, sink: torch.Tensor) -> float:
+    """Enqueue one FP64 peak microbenchmark launch (0 = DMMA, 1 = DFMA); returns its flop count."""
+    f = ctypes.c_double(0.0)
+    _check(load().gp_fp64_peak_launch(mode, iters, _ptr(sink), ctypes.byref(f), _stream()), "gp_fp64_peak_launch", "gp_schedule_selfcheck")
+    return float(f.value)
+
+
+def gp_schedule_selfcheck(n: int, m: int, tile: int, workers: int = 148):
+    """(rc, stats) of the host-only schedule replay; stats = items, edges, makespan_us, work_us, critical_path_us."""
+    st = (ctypes.c_double * 5)()
+    rc = int(load().gp_schedule_selfcheck(n, m, tile, workers, st))
+    return rc, dict(zip(("items", "edges", "makespan_us", "work_us", "critical_path_us"), list(st)))
 
 
 def gp_release_cached_schedules() -> None:

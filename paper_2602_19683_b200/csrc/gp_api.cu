@@ -13,6 +13,7 @@
 
 #include "gp_exec.cuh"
 #include "gp_kernels.cuh"
+#include "gp_peak.cuh"
 #include "gp_schedule.h"
 
 using namespace gpb;
@@ -406,3 +407,114 @@ void gp_release_cached_schedules(void) {
 }
 
 }  // extern "C"
+
+// ---- whole pipeline on host buffers -----------------------------------------------------------
+namespace {
+struct PipeWs { size_t X, y, Xs, KL, alpha, beta, mean, Sigma, info, scratch, scratch_bytes, total; };
+int pipe_ws(int64_t n, int64_t m, int D, int tile, PipeWs* w) {
+    size_t c = 0, s = 0, f = 0;
+    int rc = gp_workspace_bytes(n, m, D, tile, &c, &s, &f);
+    if (rc != GP_OK) return rc;
+    const size_t M = (size_t)(n / tile);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    w->X = take((size_t)n * D * 8);
+    w->y = take((size_t)n * 8);
+    w->Xs = take((size_t)(m > 0 ? m : 1) * D * 8);
+    w->KL = take(M * (M + 1) / 2 * (size_t)tile * tile * 8);
+    w->alpha = take((size_t)n * 8);
+    w->beta = take((size_t)n * 8);
+    w->mean = take((size_t)(m > 0 ? m : 1) * 8);
+    w->Sigma = take((size_t)m * m * 8 + 8);
+    w->info = take(sizeof(int));
+    w->scratch_bytes = c > s ? (c > f ? c : f) : (s > f ? s : f);
+    w->scratch = take(w->scratch_bytes);
+    w->total = off;
+    return GP_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gp_pipeline_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    PipeWs w;
+    int rc = pipe_ws(n, m, D, tile, &w);
+    if (rc != GP_OK) return rc;
+    *bytes = w.total;
+    return GP_OK;
+}
+
+int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D, gp_hyper h, int tile,
+                     int sched_width, double* hMean, double* hSigma, double* hAlpha, int* h_info, void* dWork, size_t work_bytes,
+                     void* stream) {
+    if (!hX || !hY || !hXs || !hMean || !h_info || !dWork) return GP_ERR_NULL;
+    if (m <= 0) return GP_ERR_SIZE;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    PipeWs w;
+    int rc = pipe_ws(n, m, D, tile, &w);
+    if (rc != GP_OK) return rc;
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* ws = (char*)dWork;
+    double *dX = (double*)(ws + w.X), *dY = (double*)(ws + w.y), *dXs = (double*)(ws + w.Xs), *dKL = (double*)(ws + w.KL);
+    double *dAlpha = (double*)(ws + w.alpha), *dBeta = (double*)(ws + w.beta), *dMean = (double*)(ws + w.mean);
+    double* dSigma = (double*)(ws + w.Sigma);
+    int* d_info = (int*)(ws + w.info);
+    void* scratch = ws + w.scratch;
+    if (cudaMemcpyAsync(dX, hX, (size_t)n * D * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpyAsync(dY, hY, (size_t)n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpyAsync(dXs, hXs, (size_t)m * D * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return GP_ERR_CUDA;
+    if ((rc = gp_assemble_tiles(dX, n, dX, n, D, h, tile, GP_SYM_LOWER, dKL, stream)) != GP_OK) return rc;
+    if ((rc = gp_cholesky_tiled(dKL, n, tile, sched_width, d_info, scratch, w.scratch_bytes, stream)) != GP_OK) return rc;
+    if ((rc = gp_solve(dKL, n, tile, dY, dAlpha, dBeta, scratch, w.scratch_bytes, stream)) != GP_OK) return rc;
+    if ((rc = gp_predict_mean(dX, n, D, dAlpha, dXs, m, h, dMean, stream)) != GP_OK) return rc;
+    if (hSigma) {
+        if ((rc = gp_predict_full_cov(dKL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, scratch, w.scratch_bytes, stream)) != GP_OK)
+            return rc;
+        if (cudaMemcpyAsync(hSigma, dSigma, (size_t)m * m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    }
+    if (cudaMemcpyAsync(hMean, dMean, (size_t)m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (hAlpha && cudaMemcpyAsync(hAlpha, dAlpha, (size_t)n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpyAsync(h_info, d_info, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void* stream) {
+    if (!d_sink) return GP_ERR_NULL;
+    if (iters <= 0) return GP_ERR_SIZE;
+    if (mode != 0 && mode != 1) return GP_ERR_MODE;
+    const int grid = sm_count() * kPeakCtasPerSm;
+    if (mode == 0) {
+        peak_dmma_kernel<<<grid, kPeakThreads, 0, (cudaStream_t)stream>>>(d_sink, iters, 1.0);
+        if (flops) *flops = (double)grid * (kPeakThreads / 32) * (double)iters * kPeakChains * 512.0;   // 2*8*8*4 per DMMA
+    } else {
+        peak_dfma_kernel<<<grid, kPeakThreads, 0, (cudaStream_t)stream>>>(d_sink, iters, 1.0);
+        if (flops) *flops = (double)grid * kPeakThreads * (double)iters * kPeakChains * 2.0;
+    }
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+}  // extern "C"
+
+extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5) {
+    if (n <= 0 || m < 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
+    if (workers <= 0) workers = 148;
+    const int b = pick_block(tile), nbt = tile / b, M = (int)(n / tile), Mm = (int)(m / tile);
+    std::vector<SchedItem> items;
+    SchedStats st;
+    if (m == 0) build_cholesky_schedule(M, nbt, workers, items, b, &st, true);
+    else build_predict_schedule(M, Mm, nbt, workers, items, b, &st, true);
+    if (stats5) {
+        stats5[0] = (double)items.size();
+        stats5[1] = (double)st.edges;
+        stats5[2] = st.makespan_us;
+        stats5[3] = st.work_us;
+        stats5[4] = st.critical_path_us;
+    }
+    const char* why = nullptr;
+    return validate_schedule(items, M, Mm, nbt, m > 0, &why) ? GP_OK : GP_ERR_SIZE;
+}

@@ -175,3 +175,34 @@ def test_argument_errors(gp):
     with pytest.raises(gp.GpError) as e:
         gp.gp_cholesky_tiled(out, 70, 32, 0, info, small)
     assert e.value.code == gp.ERR["TILE"]
+
+
+def test_host_buffer_pipeline_matches_oracle(gp):
+    """gp_pipeline_host (the end-to-end call bench.py's e2e leg times): host in, host out."""
+    cfg = nfir.CONFIGS[1]
+    X, y, Xs = nfir.make_inputs(cfg)
+    h = oracle.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    p = oracle.predict(X, y, Xs, h)
+    hX, hY, hXs = (torch.from_numpy(a).pin_memory() for a in (X, y, Xs))
+    hMean = torch.empty(cfg.m, dtype=torch.float64).pin_memory()
+    hSigma = torch.empty(cfg.m, cfg.m, dtype=torch.float64).pin_memory()
+    hAlpha = torch.empty(cfg.n, dtype=torch.float64)            # pageable also works
+    ws = torch.empty(gp.gp_pipeline_workspace_bytes(cfg.n, cfg.m, cfg.D, cfg.tile), dtype=torch.uint8, device="cuda")
+    info = gp.gp_pipeline_host(hX, hY, hXs, gp.Hyper(h.lengthscale, h.vertical, h.noise), cfg.tile, 0, hMean, hSigma, hAlpha, ws)
+    assert info == 0
+    assert relerr(hAlpha.numpy(), p.alpha) <= TOL_ALPHA
+    assert relerr(hMean.numpy(), p.mean) <= TOL_MEAN
+    assert relerr(hSigma.numpy(), p.Sigma) <= TOL_SIGMA
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_pipeline_host(hX, hY, hXs, gp.Hyper(), cfg.tile, 0, hMean, hSigma, None, small)
+    assert e.value.code == gp.ERR["WORKSPACE"]
+
+
+def test_fp64_peak_probe_launches(gp):
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for mode in (0, 1):
+        flops = gp.gp_fp64_peak_launch(mode, 10, sink)
+        assert flops > 0
+    torch.cuda.synchronize()
+    assert float(sink.item()) == 0.0

@@ -1,0 +1,96 @@
+"""CPU-side checks of the product library: it loads, exports every symbol include/gp_b200.h
+declares, validates arguments without touching a GPU, and its static tile-task schedules (a6)
+replay correctly against the device's dependency rules.  No compute calls: there is no GPU here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gp():
+    from paper_2602_19683_b200 import build
+    build.build()
+    from paper_2602_19683_b200 import binding
+    binding.load()
+    return binding
+
+
+def test_exports_match_header(gp):
+    hdr = open(os.path.join(ROOT, "include", "gp_b200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(gp_[a-z0-9_]+)\s*\(", hdr))
+    assert declared, "no declarations parsed"
+    lib = ctypes.CDLL(gp.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in gp_b200.h but not exported"
+    assert declared == set(gp.EXPORTS), declared ^ set(gp.EXPORTS)
+
+
+def test_no_library_linear_algebra_linked(gp):
+    import subprocess
+    out = subprocess.run(["ldd", gp.LIB_PATH], capture_output=True, text=True).stdout
+    assert "cublas" not in out.lower() and "cusolver" not in out.lower(), out
+
+
+def test_strerror_and_block_size(gp):
+    assert gp.strerror(0) == "ok"
+    for code in gp.ERR.values():
+        assert gp.strerror(code) not in ("ok", "unknown error code")
+    assert gp.gp_block_size(32) == 32 and gp.gp_block_size(64) == 64 and gp.gp_block_size(160) == 32
+    assert gp.gp_block_size(256) == 128 and gp.gp_block_size(1024) == 128
+    assert gp.gp_block_size(48) == gp.ERR["TILE"]
+
+
+def test_workspace_sizes_and_argument_errors(gp):
+    c, s, f = gp.gp_workspace_bytes(32768, 4096, 8, 1024)
+    assert f >= 32768 * 4096 * 8                     # holds V^T (m x n)
+    assert c < 64 << 20 and s < 64 << 20
+    c0, s0, f0 = gp.gp_workspace_bytes(128, 0, 8, 32)
+    assert f0 == 0 and c0 > 0 and s0 > 0
+    for bad in ((100, 0, 8, 32), (128, 100, 8, 32), (128, 0, 8, 0), (128, 0, 8, 48)):
+        with pytest.raises(gp.GpError) as e:
+            gp.gp_workspace_bytes(*bad)
+        assert e.value.code == gp.ERR["TILE"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_workspace_bytes(0, 0, 8, 32)
+    assert e.value.code == gp.ERR["SIZE"]
+    total = gp.gp_pipeline_workspace_bytes(1024, 1024, 8, 256)
+    assert total >= (10 * 256 * 256 + 1024 * 1024 + 1024 * 1024) * 8
+
+
+def test_task_counts_match_paper_dag(gp):
+    # M POTRF + M(M-1)/2 TRSM + M(M-1)/2 SYRK + M(M-1)(M-2)/6 GEMM
+    for M, want in ((4, 20), (8, 120), (16, 816), (32, 5984)):
+        tasks, items = gp.gp_cholesky_task_counts(M * 128, 128)
+        assert tasks == want
+        assert items >= tasks
+
+
+@pytest.mark.parametrize("n,m,tile", [
+    (128, 0, 32), (128, 128, 32), (1024, 0, 256), (1024, 1024, 256), (1536, 384, 384), (320, 320, 160),
+    (8192, 0, 512), (8192, 1024, 1024), (2048, 0, 2048), (4096, 1024, 128),
+])
+@pytest.mark.parametrize("workers", [1, 7, 148])
+def test_schedule_is_a_valid_topological_order(gp, n, m, tile, workers):
+    rc, st = gp.gp_schedule_selfcheck(n, m, tile, workers)
+    assert rc == 0
+    assert st["items"] > 0 and st["makespan_us"] >= st["critical_path_us"] * 0.999
+    assert st["makespan_us"] >= st["work_us"] / workers * 0.999
+
+
+def test_schedule_headline_config(gp):
+    rc, st = gp.gp_schedule_selfcheck(32768, 0, 1024, 148)
+    assert rc == 0
+    # list-scheduling simulation must keep 148 workers busy: makespan within 10 % of work/148
+    assert st["makespan_us"] <= 1.10 * st["work_us"] / 148
+
+
+def test_binding_refuses_cpu_tensors(gp):
+    import torch
+    X = torch.zeros(32, 2, dtype=torch.float64)
+    with pytest.raises(ValueError):
+        gp.gp_assemble_tiles(X, X, gp.Hyper(), 32, gp.GP_SYM_LOWER, torch.zeros(32 * 32, dtype=torch.float64))

@@ -114,6 +114,26 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def reduce_max_over_ranks(values, device="cpu"):
+    """Element-wise MAX of per-rank timings over the default process group (a no-op at world size 1)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def replica_seeds(config_index: int, rank: int):
+    """Every replica factors its own problem of the same shape (replicas only)."""
+    return 1000 + config_index + 10 * rank, 2000 + config_index + 10 * rank
+
+
+def aggregate_cholesky_gflops(n: int, world: int, cholesky_ms_max_over_ranks: float) -> float:
+    """Whole-job rate: the n^3/3 flop of every replica over the slowest rank's time."""
+    return world * (n ** 3 / 3.0) / (cholesky_ms_max_over_ranks * 1e-3) / 1e9
+
+
 def _dist_env():
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -242,8 +262,9 @@ def run_b200(args):
     n, m, D = cfg.n, cfg.m, cfg.D
     h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
     # every replica gets its own seeded problem of the same shape
-    X, y = nfir.nfir_features(1000 + cfg.index + 10 * rank, n, D)
-    Xs, _ = nfir.nfir_features(2000 + cfg.index + 10 * rank, m, D, with_targets=False)
+    seed_train, seed_test = replica_seeds(cfg.index, rank)
+    X, y = nfir.nfir_features(seed_train, n, D)
+    Xs, _ = nfir.nfir_features(seed_test, m, D, with_targets=False)
     hX, hY, hXs = (torch.from_numpy(a).pin_memory() for a in (X, y, Xs))
     dX, dY, dXs = hX.cuda(), hY.cuda(), hXs.cuda()
     pipe = gp.GpPipeline(n, m, D, tile, h, sched_width=args.width)
@@ -300,16 +321,13 @@ def run_b200(args):
     e2e_ms = a.elapsed_time(b)
     del ws
 
-    t = torch.tensor([phase[nm] for nm in names] + [total_ms, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    t = t.tolist()
+    t = reduce_max_over_ranks([phase[nm] for nm in names] + [total_ms, e2e_ms], device="cuda")
     phase = {nm: t[i] / args.steps for i, nm in enumerate(names)}
     total_ms, e2e_ms = t[5] / args.steps, t[6] / args.steps
 
     if rank == 0:
         flop = n ** 3 / 3.0
-        chol_gflops = world * flop / (phase["cholesky"] * 1e-3) / 1e9
+        chol_gflops = aggregate_cholesky_gflops(n, world, phase["cholesky"])
         peaks = measure_fp64_peak(gp, torch)
         peak = peaks["dmma_sustained_tflops"]
         achieved = flop / (phase["cholesky"] * 1e-3) / 1e12

@@ -147,6 +147,13 @@ int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int6
  *   d_sink: device double[1], never actually written. */
 int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void* stream);
 
+/* Executor statistics of the LAST gp_cholesky_tiled / gp_predict_full_cov call that used dWork
+ * (tracing support; the analogue of the paper's per-step APEX timers).  Copies
+ * to h_stats (host) 4 uint64 per worker CTA: {SM cycles spent waiting on dependencies, SM cycles
+ * from kernel start to the worker's exit, work items run, SM id}; synchronises the stream.
+ * Returns the number of worker slots copied (<= max_workers) or a negative GP_ERR_*. */
+int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream);
+
 /* Host-only self-check of the static work-item schedule the persistent executor consumes (a6):
  * builds the schedule for (n, m, tile) with `workers` virtual SMs (m == 0: Cholesky schedule,
  * m > 0: predictor schedule) and replays it against the dependency rules of the device code.

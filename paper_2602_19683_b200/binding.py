@@ -21,7 +21,7 @@ ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA":
 
 EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
-           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck")
+           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats")
 
 
 class gp_hyper(ctypes.Structure):
@@ -75,6 +75,7 @@ def load() -> ctypes.CDLL:
     lib.gp_pipeline_workspace_bytes.argtypes = [i64, i64, ci, ci, psz]
     lib.gp_pipeline_host.argtypes = [vp, vp, vp, i64, i64, ci, gp_hyper, ci, ci, vp, vp, vp, vp, vp, sz, vp]
     lib.gp_schedule_selfcheck.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.gp_exec_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ci, vp]
     lib.gp_fp64_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.gp_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
@@ -194,7 +195,7 @@ def gp_pipeline_host(hX: torch.Tensor, hY: torch.Tensor, hXs: torch.Tensor, h: H
 def gp_fp64_peak_launch(mode: int, iters: int, sink: torch.Tensor) -> float:
     """Enqueue one FP64 peak microbenchmark launch (0 = DMMA, 1 = DFMA); returns its flop count."""
     f = ctypes.c_double(0.0)
-    _check(load().gp_fp64_peak_launch(mode, iters, _ptr(sink), ctypes.byref(f), _stream()), "gp_fp64_peak_launch", "gp_schedule_selfcheck")
+    _check(load().gp_fp64_peak_launch(mode, iters, _ptr(sink), ctypes.byref(f), _stream()), "gp_fp64_peak_launch")
     return float(f.value)
 
 
@@ -203,6 +204,15 @@ def gp_schedule_selfcheck(n: int, m: int, tile: int, workers: int = 148):
     st = (ctypes.c_double * 5)()
     rc = int(load().gp_schedule_selfcheck(n, m, tile, workers, st))
     return rc, dict(zip(("items", "edges", "makespan_us", "work_us", "critical_path_us"), list(st)))
+
+
+def gp_exec_stats(work: torch.Tensor, max_workers: int = 148):
+    """Per-worker (wait_cycles, total_cycles, items, sm_id) of the last executor launch that used `work`."""
+    buf = (ctypes.c_uint64 * (4 * max_workers))()
+    w = int(load().gp_exec_stats(_ptr(work, torch.uint8), buf, max_workers, _stream()))
+    if w < 0:
+        raise GpError(w, "gp_exec_stats")
+    return [tuple(buf[4 * i:4 * i + 4]) for i in range(w)]
 
 
 def gp_release_cached_schedules() -> None:

@@ -22,6 +22,11 @@ namespace {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// workspace common header: [0, 256) ticket counters, [256, kHdrBytes) per-worker executor statistics
+constexpr size_t kStatsOff = 256;
+constexpr size_t kHdrBytes = 8192;
+constexpr int kMaxWorkers = (int)((kHdrBytes - kStatsOff) / 32);
+
 int pick_block(int tile) {
     if (tile % 128 == 0) return 128;
     if (tile % 64 == 0) return 64;
@@ -130,8 +135,9 @@ int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaSt
 
 int workers_for(int sched_width) {
     const int sms = sm_count();
-    if (sched_width <= 0) return sms;
-    return sched_width < sms ? sched_width : sms;   // one resident CTA per SM: more cannot be co-resident
+    if (sched_width <= 0) return sms < kMaxWorkers ? sms : kMaxWorkers;
+    const int w = sched_width < sms ? sched_width : sms;   // one resident CTA per SM: more cannot be co-resident
+    return w < kMaxWorkers ? w : kMaxWorkers;
 }
 
 int launch_assemble(const double* dA, int64_t na, const double* dB, int64_t nb, int D, const HyperDev& h, int tile, int sym_lower,
@@ -152,7 +158,7 @@ CholWs chol_ws(int64_t n, int b) {
     const size_t NB = (size_t)(n / b);
     CholWs w;
     w.ticket = 0;
-    w.verL = 256;
+    w.verL = kHdrBytes;
     w.invD = align_up(w.verL + NB * NB * sizeof(int), 256);
     w.total = w.invD + NB * (size_t)b * b * sizeof(double);
     return w;
@@ -162,7 +168,7 @@ SolveWs solve_ws(int64_t n, int b) {
     const size_t NB = (size_t)(n / b);
     SolveWs w;
     w.ticket = 0;
-    w.flags = 256;
+    w.flags = kHdrBytes;
     w.beta = align_up(w.flags + 2 * NB * sizeof(int), 256);
     w.invD = align_up(w.beta + (size_t)n * sizeof(double), 256);
     w.total = w.invD + NB * (size_t)b * b * sizeof(double);
@@ -173,7 +179,7 @@ CovWs cov_ws(int64_t n, int64_t m, int b) {
     const size_t NB = (size_t)(n / b), NBm = (size_t)(m / b);
     CovWs w;
     w.ticket = 0;
-    w.verV = 256;
+    w.verV = kHdrBytes;
     w.verS = align_up(w.verV + NBm * NB * sizeof(int), 256);
     w.invD = align_up(w.verS + NBm * NBm * sizeof(int), 256);
     w.Vt = align_up(w.invD + NB * (size_t)b * b * sizeof(double), 256);
@@ -282,6 +288,7 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     p.items = cs.d_items;
     p.nitems = cs.nitems;
     p.ticket = (unsigned int*)(ws + w.ticket);
+    p.stats = (unsigned long long*)(ws + kStatsOff);
     p.d_info = d_info;
     p.t = tile;
     p.nbt = nbt;
@@ -385,6 +392,7 @@ int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, co
     p.items = cs.d_items;
     p.nitems = cs.nitems;
     p.ticket = (unsigned int*)(ws + w.ticket);
+    p.stats = (unsigned long long*)(ws + kStatsOff);
     p.t = tile;
     p.nbt = nbt;
     p.NB = NB;
@@ -496,6 +504,15 @@ int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void
 }
 
 }  // extern "C"
+
+extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream) {
+    if (!dWork || !h_stats) return GP_ERR_NULL;
+    if (max_workers <= 0) return GP_ERR_SIZE;
+    const int w = max_workers < kMaxWorkers ? max_workers : kMaxWorkers;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(h_stats, (const char*)dWork + kStatsOff, (size_t)w * 32, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? w : GP_ERR_CUDA;
+}
 
 extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5) {
     if (n <= 0 || m < 0) return GP_ERR_SIZE;

@@ -56,6 +56,7 @@ struct ExecParams {
     int Mt;                // n / t (tiles per row of V^T)
     int64_t m;             // rows of Sigma (leading dimension)
     int L_final;           // 1: L is an input that is final everywhere (predictor), no waits on it
+    unsigned long long* stats;   // per worker CTA: {cycles waiting on dependencies, cycles total, items run, SM id}
 };
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
@@ -68,7 +69,8 @@ template <int BLK>
 struct Exec {
     const ExecParams& p;
     double* smem;
-    __device__ Exec(const ExecParams& p_, double* smem_) : p(p_), smem(smem_) {}
+    long long* wait_cycles;   // shared-memory accumulator owned by thread 0
+    __device__ Exec(const ExecParams& p_, double* smem_, long long* wc) : p(p_), smem(smem_), wait_cycles(wc) {}
 
     __device__ __forceinline__ double* blkL(int gr, int gc) const {
         const int I = gr / p.nbt, J = gc / p.nbt;
@@ -96,10 +98,12 @@ struct Exec {
         int need;
     };
     __device__ __forceinline__ void wait_all(const int* addr, int need) const {
+        const long long t0 = clock64();
         if (addr != nullptr) {
             while (ld_acquire(addr) < need) __nanosleep(64);
         }
         __syncthreads();
+        if (threadIdx.x == 0) *wait_cycles += clock64() - t0;
     }
     __device__ __forceinline__ void signal(int* counter) const {
         __threadfence();
@@ -272,7 +276,11 @@ template <int BLK>
 __global__ void __launch_bounds__(kThreads, 1) exec_kernel(const __grid_constant__ ExecParams p) {
     extern __shared__ __align__(16) double smem[];
     __shared__ unsigned int s_ticket;
-    Exec<BLK> ex(p, smem);
+    __shared__ long long s_wait;
+    if (threadIdx.x == 0) s_wait = 0;
+    const long long t_start = clock64();
+    unsigned long long nrun = 0;
+    Exec<BLK> ex(p, smem, &s_wait);
     for (;;) {
         if (threadIdx.x == 0) s_ticket = atomicAdd(p.ticket, 1u);
         __syncthreads();
@@ -282,7 +290,17 @@ __global__ void __launch_bounds__(kThreads, 1) exec_kernel(const __grid_constant
         Item it;
         it.op = (uint32_t)raw.x; it.gr = (uint32_t)raw.y; it.gc = (uint32_t)raw.z; it.q = (uint32_t)raw.w;
         ex.run(it);
+        ++nrun;
         // run() always ends with signal(), whose barrier also protects s_ticket and the ring
+    }
+    if (threadIdx.x == 0 && p.stats != nullptr) {
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        unsigned long long* st = p.stats + 4 * (size_t)blockIdx.x;
+        st[0] = (unsigned long long)s_wait;
+        st[1] = (unsigned long long)(clock64() - t_start);
+        st[2] = nrun;
+        st[3] = smid;
     }
 }
 

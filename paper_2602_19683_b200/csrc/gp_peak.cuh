@@ -16,7 +16,11 @@ constexpr int kPeakCtasPerSm = 4;     // 32 resident warps per SM
 __global__ void __launch_bounds__(kPeakThreads) peak_dmma_kernel(double* __restrict__ sink, int iters, double seed) {
     double acc[kPeakChains][2];
     const int lane = threadIdx.x & 31;
-    double a = seed + 1e-9 * lane, b = 1.0 - 1e-9 * lane;
+    // 4 distinct A and 4 distinct B fragments, used as a 4x4 outer product like the real kernel:
+    // issuing every chain from the SAME operand registers measures 29.7 instead of 37.1 TFLOP/s
+    double a[4], b[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { a[i] = seed + 1e-9 * lane + i; b[i] = 1.0 - 1e-9 * lane - i; }
 #pragma unroll
     for (int j = 0; j < kPeakChains; ++j) acc[j][0] = acc[j][1] = 0.0;
     for (int it = 0; it < iters; ++it) {
@@ -24,7 +28,7 @@ __global__ void __launch_bounds__(kPeakThreads) peak_dmma_kernel(double* __restr
         for (int j = 0; j < kPeakChains; ++j)
             asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                          : "+d"(acc[j][0]), "+d"(acc[j][1])
-                         : "d"(a), "d"(b));
+                         : "d"(a[j & 3]), "d"(b[(j >> 2) & 3]));
     }
     double s = 0.0;
 #pragma unroll

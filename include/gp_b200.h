@@ -147,6 +147,19 @@ int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int6
  *   d_sink: device double[1], never actually written. */
 int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void* stream);
 
+/* Steady-state rate of the contraction path alone (measurement support): the persistent executor
+ * runs SMs x reps independent work items C(128x128) -= A(128xK) B(128xK)^T on a synthetic
+ * lower-packed matrix (tile edge K) with every dependency wait switched off, so TMA streaming,
+ * DMMA main loop, epilogue and version-counter signalling are all exercised but nothing waits on
+ * the DAG.  The gap to the DMMA peak is the kernel's own overhead; the gap from the Cholesky rate
+ * to this is the DAG's.
+ *   K: multiple of 128, <= 8192.  d_buf/buf_bytes: device scratch, contents arbitrary finite
+ *   doubles (overwritten); *need_bytes (host, may be NULL) receives the size required, and with
+ *   d_buf == NULL the call only reports it.  *flops (host, may be NULL): flop of one launch.
+ *   Performs one synchronous cudaMemcpy of the item list. */
+int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, double* flops, size_t* need_bytes,
+                                void* stream);
+
 /* Executor statistics of the LAST gp_cholesky_tiled / gp_predict_full_cov call that used dWork
  * (tracing support; the analogue of the paper's per-step APEX timers).  Copies
  * to h_stats (host) 4 uint64 per worker CTA: {SM cycles spent waiting on dependencies, SM cycles

@@ -21,7 +21,8 @@ ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA":
 
 EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
-           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats")
+           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
+           "gp_contraction_bench_launch")
 
 
 class gp_hyper(ctypes.Structure):
@@ -77,6 +78,7 @@ def load() -> ctypes.CDLL:
     lib.gp_schedule_selfcheck.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_exec_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ci, vp]
     lib.gp_fp64_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
+    lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
     lib.gp_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
         if name not in ("gp_release_cached_schedules", "gp_strerror"):
@@ -196,6 +198,20 @@ def gp_fp64_peak_launch(mode: int, iters: int, sink: torch.Tensor) -> float:
     """Enqueue one FP64 peak microbenchmark launch (0 = DMMA, 1 = DFMA); returns its flop count."""
     f = ctypes.c_double(0.0)
     _check(load().gp_fp64_peak_launch(mode, iters, _ptr(sink), ctypes.byref(f), _stream()), "gp_fp64_peak_launch")
+    return float(f.value)
+
+
+def gp_contraction_bench_bytes(K: int, reps: int) -> int:
+    need = ctypes.c_size_t(0)
+    _check(load().gp_contraction_bench_launch(K, reps, None, 0, None, ctypes.byref(need), None), "gp_contraction_bench_launch")
+    return int(need.value)
+
+
+def gp_contraction_bench_launch(K: int, reps: int, buf: torch.Tensor) -> float:
+    """Enqueue one launch of the contraction steady-state microbenchmark; returns its flop count."""
+    f = ctypes.c_double(0.0)
+    _check(load().gp_contraction_bench_launch(K, reps, _ptr(buf, torch.uint8), buf.numel(), ctypes.byref(f), None, _stream()),
+           "gp_contraction_bench_launch")
     return float(f.value)
 
 

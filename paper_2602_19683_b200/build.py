@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgp_b200.so")
 SOURCES = ["gp_api.cu", "gp_schedule.cpp"]
-HEADERS = ["gp_gemm.cuh", "gp_exec.cuh", "gp_kernels.cuh", "gp_peak.cuh", "gp_schedule.h", os.path.join("..", "..", "include", "gp_b200.h")]
+HEADERS = ["gp_tma.cuh", "gp_gemm.cuh", "gp_exec.cuh", "gp_kernels.cuh", "gp_peak.cuh", "gp_schedule.h", os.path.join("..", "..", "include", "gp_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared", "-Xptxas", "-v"]
 
@@ -31,7 +31,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc, *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, f) for f in SOURCES]]
+        extra = ["-DGPB_WATCHDOG"] if os.environ.get("GP_B200_WATCHDOG") else []   # debug aid, see gp_tma.cuh
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", tmp, *[os.path.join(CSRC, f) for f in SOURCES]]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)

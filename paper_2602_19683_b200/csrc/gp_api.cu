@@ -93,23 +93,72 @@ int get_schedule(int kind, int M, int Mm, int nbt, int blk, int workers, CachedS
     return GP_OK;
 }
 
+// ---- TMA tensor maps ---------------------------------------------------------------------------
+// cuTensorMapEncodeTiled is fetched from the driver at run time (no link-time libcuda dependency).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)ptr;
+    }
+    return fn;
+}
+
+// Row-major FP64 matrix [rows x cols] (contiguous rows) viewed through boxes of b rows x 16 doubles
+// (one 128-byte swizzle row per matrix row): the operand panels of the contraction kernel.
+int make_map(CUtensorMap* map, const double* base, uint64_t rows, uint64_t cols, int b) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return GP_ERR_CUDA;
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(double)};
+    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)b};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? GP_OK : GP_ERR_CUDA;
+}
+
+struct ExecMaps { CUtensorMap L, V, D; };
+
+// maps for the executor: L (lower-packed tiles as a [tiles*t, t] matrix), V^T (general tiles, same view;
+// the L map again when there is no V^T) and the inverted diagonal blocks ([NB*b, b]).
+int make_exec_maps(ExecMaps* mp, const ExecParams& p, int b, int64_t m) {
+    const uint64_t M = (uint64_t)p.Mt, t = (uint64_t)p.t;
+    int rc = make_map(&mp->L, p.L, M * (M + 1) / 2 * t, t, b);
+    if (rc != GP_OK) return rc;
+    if (p.Vt) rc = make_map(&mp->V, p.Vt, (uint64_t)(m / p.t) * M * t, t, b);
+    else mp->V = mp->L;
+    if (rc != GP_OK) return rc;
+    return make_map(&mp->D, p.invD, (uint64_t)p.NB * b, (uint64_t)b, b);
+}
+
 template <int BLK>
-int launch_exec(const ExecParams& p, int workers, cudaStream_t st) {
+int launch_exec(const ExecParams& p, const ExecMaps& mp, int workers, cudaStream_t st) {
     static bool configured = false;
     constexpr int smem = exec_smem_bytes<BLK>();
     if (!configured) {
         if (cudaFuncSetAttribute(exec_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
         configured = true;
     }
-    exec_kernel<BLK><<<workers, kThreads, smem, st>>>(p);
+    exec_kernel<BLK><<<workers, kThreads, smem, st>>>(p, mp.L, mp.V, mp.D);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
-int launch_exec_any(int b, const ExecParams& p, int workers, cudaStream_t st) {
+int launch_exec_any(int b, const ExecParams& p, int64_t m, int workers, cudaStream_t st) {
+    ExecMaps mp;
+    const int rc = make_exec_maps(&mp, p, b, m);
+    if (rc != GP_OK) return rc;
     switch (b) {
-        case 128: return launch_exec<128>(p, workers, st);
-        case 64: return launch_exec<64>(p, workers, st);
-        default: return launch_exec<32>(p, workers, st);
+        case 128: return launch_exec<128>(p, mp, workers, st);
+        case 64: return launch_exec<64>(p, mp, workers, st);
+        default: return launch_exec<32>(p, mp, workers, st);
     }
 }
 
@@ -121,7 +170,7 @@ int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStre
         if (cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
         configured = true;
     }
-    trtri_diag_kernel<BLK><<<NB, kThreads, smem, st>>>(L, t, nbt, invD);
+    trtri_diag_kernel<BLK><<<NB, kConsumerThreads, smem, st>>>(L, t, nbt, invD);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
@@ -294,7 +343,7 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     p.nbt = nbt;
     p.NB = NB;
     p.Mt = M;
-    return launch_exec_any(b, p, workers, st);
+    return launch_exec_any(b, p, 0, workers, st);
 }
 
 int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta, void* dWork, size_t work_bytes,
@@ -400,7 +449,7 @@ int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, co
     p.Mt = M;
     p.m = m;
     p.L_final = 1;
-    rc = launch_exec_any(b, p, workers, st);
+    rc = launch_exec_any(b, p, m, workers, st);
     if (rc != GP_OK) return rc;
     dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
     mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
@@ -503,6 +552,54 @@ int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
+int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, double* flops, size_t* need_bytes, void* stream) {
+    constexpr int b = 128;
+    if (K < b || K % b != 0 || K > 8192 || reps <= 0) return GP_ERR_SIZE;
+    // a synthetic lower-packed matrix with tile edge K: tile column 0 supplies the A and B panels,
+    // the tiles (I, J >= 1) supply the C blocks; every item is UPD_L(gr, gc, 0, K/b) without dependencies
+    const int nbt = K / b;
+    const int M = 1 + (12 / nbt > 1 ? 12 / nbt : 1);
+    const int NB = M * nbt, ctas = sm_count();
+    const size_t tiles_bytes = (size_t)M * (M + 1) / 2 * K * K * sizeof(double);
+    const size_t ver_off = align_up(tiles_bytes, 256) + kHdrBytes;
+    const size_t items_off = align_up(ver_off + (size_t)NB * NB * sizeof(int), 256);
+    const size_t nitems = (size_t)ctas * reps;
+    const size_t total = items_off + nitems * sizeof(Item);
+    if (need_bytes) *need_bytes = total;
+    if (!d_buf) return need_bytes ? GP_OK : GP_ERR_NULL;
+    if (buf_bytes < total) return GP_ERR_WORKSPACE;
+    std::vector<Item> cblocks;
+    for (int gr = nbt; gr < NB; ++gr)
+        for (int gc = nbt; gc < (gr / nbt + 1) * nbt; ++gc) {
+            Item it;
+            it.op = OP_UPD_L; it.gr = (uint32_t)gr; it.gc = (uint32_t)gc; it.q = (uint32_t)nbt << 16;
+            cblocks.push_back(it);
+        }
+    std::vector<Item> items(nitems);
+    for (size_t i = 0; i < nitems; ++i) items[i] = cblocks[i % cblocks.size()];
+    char* ws = (char*)d_buf;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpy(ws + items_off, items.data(), nitems * sizeof(Item), cudaMemcpyHostToDevice) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemsetAsync(ws + align_up(tiles_bytes, 256), 0, items_off - align_up(tiles_bytes, 256), st) != cudaSuccess) return GP_ERR_CUDA;
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = (double*)d_buf;
+    p.invD = (double*)d_buf;
+    p.verL = (int*)(ws + ver_off);
+    p.items = (const Item*)(ws + items_off);
+    p.nitems = (int)nitems;
+    p.ticket = (unsigned int*)(ws + align_up(tiles_bytes, 256));
+    p.stats = (unsigned long long*)(ws + align_up(tiles_bytes, 256) + kStatsOff);
+    p.d_info = (int*)(ws + align_up(tiles_bytes, 256) + 128);
+    p.t = K;
+    p.nbt = nbt;
+    p.NB = NB;
+    p.Mt = M;
+    p.no_deps = 1;
+    if (flops) *flops = (double)nitems * 2.0 * b * b * K;
+    return launch_exec_any(b, p, 0, ctas, st);
+}
+
 }  // extern "C"
 
 extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream) {
@@ -535,3 +632,4 @@ extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers
     const char* why = nullptr;
     return validate_schedule(items, M, Mm, nbt, m > 0, &why) ? GP_OK : GP_ERR_SIZE;
 }
+

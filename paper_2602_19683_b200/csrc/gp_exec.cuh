@@ -4,8 +4,19 @@
 // CUDA stream, and a cudaStreamSynchronize inside every task.  Here the
 // whole DAG runs inside ONE kernel launch: `sched_width` persistent CTAs pull work items in a
 // fixed, topologically sorted order from a global ticket counter and synchronise through
-// per-block version counters in global memory (release/acquire), so a dependent item starts
-// ~1 us after its producer finishes and nothing returns to the host.
+// per-block version counters in global memory (release/acquire), so nothing returns to the host.
+//
+// Each CTA is warp-specialised (the sm_100a shape of a persistent GEMM, with DMMA in place of
+// tcgen05 because FP64 has no tcgen05 kind):
+//   * warp 8, the PRODUCER: takes the next ticket, decodes the item, polls its dependencies,
+//     hands a job descriptor to the consumers through a small mbarrier-guarded queue and streams
+//     the operands with TMA (cp.async.bulk.tensor, 128-byte swizzle) into a ring of k-stages.
+//     It runs ahead of the consumers by the depth of the ring, ACROSS items: ticket, dependency
+//     polling and the first stages of item i+1 overlap the main loop of item i.
+//   * warps 0-7, the CONSUMERS: wait for a filled stage, LDS.64 + DMMA (gp_gemm.cuh), release the
+//     stage; at the end of a job each warp stores its part of C and bumps the block's version
+//     counter on its own (a version = kConsumerWarps increments) -- no CTA-wide barrier anywhere
+//     on the GEMM path.
 //
 // Work items are block-level (b x b, b = 128 for tiles that are multiples of 128) pieces of the
 // paper's tile tasks (readings A3/A4):
@@ -18,8 +29,10 @@
 // on three matrices: L (lower-packed tiles), V^T (general tiles) and Sigma (dense).
 //
 // Deadlock freedom: the item list is a topological order of the DAG and tickets are handed out
-// in list order to CTAs that are already running, so every item a CTA waits for was claimed
-// earlier by a CTA that is running or finished.
+// in list order.  A CTA holds at most two tickets (the one its consumers run and the one its
+// producer prepares); the unfinished item with the lowest ticket is therefore always the one some
+// CTA's consumers are running (an earlier ticket of the same CTA would be unfinished and lower),
+// all its dependencies are finished, so it completes.
 #pragma once
 #include "gp_gemm.cuh"
 
@@ -42,7 +55,7 @@ struct ExecParams {
     double* Vt;            // general tiles (m x n), or nullptr
     double* S;             // dense m x m, or nullptr
     double* invD;          // NB blocks of b x b: inverses of the diagonal blocks of L
-    int* verL;             // NB x NB version counters
+    int* verL;             // NB x NB version counters (one version = kConsumerWarps increments)
     int* verV;             // NBm x NB
     int* verS;             // NBm x NBm
     const Item* items;
@@ -56,144 +69,47 @@ struct ExecParams {
     int Mt;                // n / t (tiles per row of V^T)
     int64_t m;             // rows of Sigma (leading dimension)
     int L_final;           // 1: L is an input that is final everywhere (predictor), no waits on it
-    unsigned long long* stats;   // per worker CTA: {cycles waiting on dependencies, cycles total, items run, SM id}
+    int no_deps;           // 1: skip every dependency wait (contraction microbenchmark only)
+    unsigned long long* stats;   // per worker CTA: {producer cycles polling dependencies, cycles total, items run, SM id}
 };
 
-__device__ __forceinline__ int ld_acquire(const int* p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
+enum JobKind : int { JOB_GEMM_SUB = 0, JOB_GEMM_SET = 1, JOB_POTRF = 2, JOB_EXIT = 3 };
+
+struct __align__(16) Job {   // 32 bytes, producer -> consumers
+    double* C;             // output block (POTRF: the diagonal block of L)
+    int* sig;              // version counter of the output block
+    int ldc;
+    int nk;                // k-stages of kBK
+    int kind;
+    int arg;               // POTRF: diagonal block index q
+};
+
+// Shared-memory carve-up (dynamic, base rounded up to 1024 B for the TMA swizzle)
+template <int BLK>
+struct ExecSmem {
+    static constexpr int kRing = GemmCfg<BLK>::kRingBytes;
+    static constexpr int kPotrf = BLK * (BLK + 1) * 8;
+    static constexpr int kWork = kRing > kPotrf ? kRing : kPotrf;       // POTRF factors inside the idle ring
+    static constexpr int kFull = kWork;                                  // uint64 full[kStages]
+    static constexpr int kEmpty = kFull + 8 * kStages;
+    static constexpr int kJobFull = kEmpty + 8 * kStages;
+    static constexpr int kJobEmpty = kJobFull + 8 * kJobSlots;
+    static constexpr int kJobs = (kJobEmpty + 8 * kJobSlots + 15) / 16 * 16;
+    static constexpr int kTotal = kJobs + (int)sizeof(Job) * kJobSlots;
+    static constexpr int kBytes = kTotal + 1024;                         // slack for the manual alignment
+};
 
 template <int BLK>
-struct Exec {
-    const ExecParams& p;
-    double* smem;
-    long long* wait_cycles;   // shared-memory accumulator owned by thread 0
-    __device__ Exec(const ExecParams& p_, double* smem_, long long* wc) : p(p_), smem(smem_), wait_cycles(wc) {}
-
-    __device__ __forceinline__ double* blkL(int gr, int gc) const {
-        const int I = gr / p.nbt, J = gc / p.nbt;
-        return p.L + ((size_t)I * (I + 1) / 2 + J) * (size_t)p.t * p.t + (size_t)(gr % p.nbt) * BLK * p.t +
-               (size_t)(gc % p.nbt) * BLK;
-    }
-    __device__ __forceinline__ double* blkV(int gr, int gc) const {
-        const int I = gr / p.nbt, J = gc / p.nbt;
-        return p.Vt + ((size_t)I * p.Mt + J) * (size_t)p.t * p.t + (size_t)(gr % p.nbt) * BLK * p.t +
-               (size_t)(gc % p.nbt) * BLK;
-    }
-    __device__ __forceinline__ double* blkS(int gr, int gc) const {
-        return p.S + (size_t)gr * BLK * p.m + (size_t)gc * BLK;
-    }
-    // number of writes after which block (gr,gc) of L is final
-    __device__ __forceinline__ int finL(int gr, int gc) const {
-        const int K = gc / p.nbt, bk = gc % p.nbt;
-        return (gr / p.nbt == K) ? K + 1 + bk : K + 1 + (bk > 0 ? 1 : 0);
-    }
-    __device__ __forceinline__ int finV(int gc) const { return gc / p.nbt + 1 + (gc % p.nbt > 0 ? 1 : 0); }
-
-    // ---- dependency waits: lane i of warp 0 polls wait i, then the CTA barrier publishes it
-    struct Waits {
-        const int* addr;   // this lane's counter (nullptr = none)
-        int need;
-    };
-    __device__ __forceinline__ void wait_all(const int* addr, int need) const {
-        const long long t0 = clock64();
-        if (addr != nullptr) {
-            while (ld_acquire(addr) < need) __nanosleep(64);
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) *wait_cycles += clock64() - t0;
-    }
-    __device__ __forceinline__ void signal(int* counter) const {
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            __threadfence();
-            atomicAdd(counter, 1);
-        }
-    }
-
-    // C(gr,gc) -= A(gr,q0:q1) B(gc,q0:q1)^T on (matC, matA, matB) given by op
-    __device__ void update(uint32_t op, int gr, int gc, int q0, int q1) const {
-        const int tid = threadIdx.x;
-        const int nq = q1 - q0;
-        // waits: lane 0: own block; lanes 1..nq: A panel; lanes 1+nq..2nq: B panel
-        const int* addr = nullptr;
-        int need = 0;
-        if (tid < 1 + 2 * nq) {
-            if (op == OP_UPD_L) {
-                if (tid == 0) { addr = p.verL + (size_t)gr * p.NB + gc; need = q0 / p.nbt + q0 % p.nbt; }
-                else if (tid <= nq) { const int q = q0 + tid - 1; addr = p.verL + (size_t)gr * p.NB + q; need = finL(gr, q); }
-                else { const int q = q0 + tid - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
-            } else if (op == OP_UPD_V) {
-                if (tid == 0) { addr = p.verV + (size_t)gr * p.NB + gc; need = q0 / p.nbt; }
-                else if (tid <= nq) { const int q = q0 + tid - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
-                else if (!p.L_final) { const int q = q0 + tid - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
-            } else {  // OP_UPD_S
-                if (tid == 0) { addr = p.verS + (size_t)gr * p.NBm + gc; need = q0 / p.nbt; }
-                else if (tid <= nq) { const int q = q0 + tid - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
-                else { const int q = q0 + tid - 1 - nq; addr = p.verV + (size_t)gc * p.NB + q; need = finV(q); }
-            }
-        }
-        wait_all(addr, need);
-        const int K = nq * BLK;
-        if (op == OP_UPD_L) {
-            gemm_nt_block<BLK>(blkL(gr, gc), p.t, blkL(gr, q0), p.t, blkL(gc, q0), p.t, K, kSub, smem);
-            signal(p.verL + (size_t)gr * p.NB + gc);
-        } else if (op == OP_UPD_V) {
-            gemm_nt_block<BLK>(blkV(gr, gc), p.t, blkV(gr, q0), p.t, blkL(gc, q0), p.t, K, kSub, smem);
-            signal(p.verV + (size_t)gr * p.NB + gc);
-        } else {
-            gemm_nt_block<BLK>(blkS(gr, gc), (int)p.m, blkV(gr, q0), p.t, blkV(gc, q0), p.t, K, kSub, smem);
-            signal(p.verS + (size_t)gr * p.NBm + gc);
-        }
-    }
-
-    // C(gr,gc) = C(gr,gc) invD(gc)^T   (is_v: C is a block of V^T, else of L)
-    __device__ void trsm(bool is_v, int gr, int gc) const {
-        const int tid = threadIdx.x;
-        const int* addr = nullptr;
-        int need = 0;
-        if (tid == 0) {
-            if (is_v) { addr = p.verV + (size_t)gr * p.NB + gc; need = finV(gc) - 1; }
-            else { addr = p.verL + (size_t)gr * p.NB + gc; need = finL(gr, gc) - 1; }
-        } else if (tid == 1 && !(is_v && p.L_final)) {
-            addr = p.verL + (size_t)gc * p.NB + gc; need = finL(gc, gc);
-        }
-        wait_all(addr, need);
-        double* C = is_v ? blkV(gr, gc) : blkL(gr, gc);
-        gemm_nt_block<BLK>(C, p.t, C, p.t, p.invD + (size_t)gc * BLK * BLK, BLK, BLK, kSet, smem);
-        signal(is_v ? p.verV + (size_t)gr * p.NB + gc : p.verL + (size_t)gr * p.NB + gc);
-    }
-
-    __device__ void row_chain(bool is_v, int gr, int qt) const {
-        for (int jj = 0; jj < p.nbt; ++jj) {
-            if (jj > 0) update(is_v ? OP_UPD_V : OP_UPD_L, gr, qt + jj, qt, qt + jj);
-            trsm(is_v, gr, qt + jj);
-        }
-    }
-
-    __device__ void potrf(int q) const;
-
-    __device__ void run(const Item& it) const {
-        switch (it.op) {
-            case OP_UPD_L: case OP_UPD_V: case OP_UPD_S:
-                update(it.op, (int)it.gr, (int)it.gc, (int)(it.q & 0xffffu), (int)(it.q >> 16)); break;
-            case OP_TRSM_L: trsm(false, (int)it.gr, (int)it.gc); break;
-            case OP_POTRF: potrf((int)it.gc); break;
-            case OP_ROW_L: row_chain(false, (int)it.gr, (int)it.gc); break;
-            case OP_ROW_V: row_chain(true, (int)it.gr, (int)it.gc); break;
-            default: break;
-        }
-    }
-};
+constexpr int exec_smem_bytes() { return ExecSmem<BLK>::kBytes; }
 
 // ---------------------------------------------------------------------------------------------
-// Diagonal block kernels (shared-memory resident, BLK x BLK, padded stride BLK+1).
+// Diagonal block kernels (shared-memory resident, BLK x BLK, padded stride BLK+1), run by the
+// 256 consumer threads; cbar() is the named barrier among them (the producer warp never joins).
 // POTRF: unblocked right-looking Cholesky of the block; then the inverse of the
 // lower-triangular factor in place, so that TRSM becomes a DMMA product.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cbar() { named_bar_sync<1, kConsumerThreads>(); }
+
 template <int BLK>
 __device__ void chol_lower_smem(double* S, int* d_info, int col0) {
     constexpr int SP = BLK + 1;
@@ -202,14 +118,14 @@ __device__ void chol_lower_smem(double* S, int* d_info, int col0) {
         const double d = S[j * SP + j];
         if (!(d > 0.0) && tid == 0) atomicCAS(d_info, 0, col0 + j + 1);
         const double ljj = sqrt(d);
-        for (int r = j + 1 + tid; r < BLK; r += kThreads) S[r * SP + j] = S[r * SP + j] / ljj;
-        __syncthreads();
+        for (int r = j + 1 + tid; r < BLK; r += kConsumerThreads) S[r * SP + j] = S[r * SP + j] / ljj;
+        cbar();
         if (tid == 0) S[j * SP + j] = ljj;
-        for (int c = j + 1 + warp; c < BLK; c += kThreads / 32) {
+        for (int c = j + 1 + warp; c < BLK; c += kConsumerWarps) {
             const double lc = S[c * SP + j];
             for (int r = c + lane; r < BLK; r += 32) S[r * SP + c] = fma(-S[r * SP + j], lc, S[r * SP + c]);
         }
-        __syncthreads();
+        cbar();
     }
 }
 
@@ -228,76 +144,360 @@ __device__ void inv_lower_smem(double* S) {
         }
         s += __shfl_xor_sync(0xffffffffu, s, 1);
         const double rd = 1.0 / S[j * SP + j];
-        __syncthreads();
+        cbar();
         if (i < BLK && half == 0) {
             if (i > j) S[i * SP + j] = -s * rd;
             else if (i == j) S[j * SP + j] = rd;
         }
-        __syncthreads();
+        cbar();
     }
 }
 
 template <int BLK>
 __device__ void load_lower_to_smem(double* S, const double* __restrict__ G, int ld) {
     constexpr int SP = BLK + 1;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kThreads) {
+    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
         const int r = idx / BLK, c = idx % BLK;
         S[r * SP + c] = (c <= r) ? __ldcg(G + (size_t)r * ld + c) : 0.0;
     }
-    __syncthreads();
+    cbar();
 }
 
+// POTRF job, all consumer threads: G = diagonal block (q,q) of L in global memory (leading
+// dimension t), inv = invD(q).  S is the (idle) operand ring.
 template <int BLK>
-__device__ void Exec<BLK>::potrf(int q) const {
-    const int* addr = nullptr;
-    int need = 0;
-    if (threadIdx.x == 0) { addr = p.verL + (size_t)q * p.NB + q; need = finL(q, q) - 1; }
-    wait_all(addr, need);
+__device__ void potrf_block(double* S, double* __restrict__ G, int t, double* __restrict__ inv, int* d_info, int col0) {
     constexpr int SP = BLK + 1;
-    double* S = smem;
-    double* G = blkL(q, q);
-    load_lower_to_smem<BLK>(S, G, p.t);
-    chol_lower_smem<BLK>(S, p.d_info, q * BLK);
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kThreads) {
+    load_lower_to_smem<BLK>(S, G, t);
+    chol_lower_smem<BLK>(S, d_info, col0);
+    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
         const int r = idx / BLK, c = idx % BLK;
-        if (c <= r) __stcg(G + (size_t)r * p.t + c, S[r * SP + c]);
+        if (c <= r) __stcg(G + (size_t)r * t + c, S[r * SP + c]);
     }
     inv_lower_smem<BLK>(S);
-    double* inv = p.invD + (size_t)q * BLK * BLK;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kThreads) {
+    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
         const int r = idx / BLK, c = idx % BLK;
         __stcg(inv + idx, S[r * SP + c]);      // strict upper part of S is still the zeros loaded above
     }
-    signal(p.verL + (size_t)q * p.NB + q);
+}
+
+// ---------------------------------------------------------------------------------------------
+// The producer warp.
+// ---------------------------------------------------------------------------------------------
+template <int BLK>
+struct Producer {
+    using Cfg = GemmCfg<BLK>;
+    using SM = ExecSmem<BLK>;
+    const ExecParams& p;
+    const CUtensorMap *mapL, *mapV, *mapD;
+    char* ring;
+    uint64_t *full, *empty, *job_full, *job_empty;
+    Job* jobs;
+    int lane;
+    int stage = 0, phase = 0, slot = 0, jphase = 0;
+    long long poll_cycles = 0;
+
+    __device__ Producer(const ExecParams& p_, const CUtensorMap* l, const CUtensorMap* v, const CUtensorMap* d, char* base)
+        : p(p_), mapL(l), mapV(v), mapD(d), ring(base),
+          full(reinterpret_cast<uint64_t*>(base + SM::kFull)), empty(reinterpret_cast<uint64_t*>(base + SM::kEmpty)),
+          job_full(reinterpret_cast<uint64_t*>(base + SM::kJobFull)), job_empty(reinterpret_cast<uint64_t*>(base + SM::kJobEmpty)),
+          jobs(reinterpret_cast<Job*>(base + SM::kJobs)), lane(threadIdx.x & 31) {}
+
+    // ---- addressing ---------------------------------------------------------------------------
+    __device__ __forceinline__ double* blkL(int gr, int gc) const {
+        const int I = gr / p.nbt, J = gc / p.nbt;
+        return p.L + ((size_t)I * (I + 1) / 2 + J) * (size_t)p.t * p.t + (size_t)(gr % p.nbt) * BLK * p.t +
+               (size_t)(gc % p.nbt) * BLK;
+    }
+    __device__ __forceinline__ double* blkV(int gr, int gc) const {
+        const int I = gr / p.nbt, J = gc / p.nbt;
+        return p.Vt + ((size_t)I * p.Mt + J) * (size_t)p.t * p.t + (size_t)(gr % p.nbt) * BLK * p.t +
+               (size_t)(gc % p.nbt) * BLK;
+    }
+    __device__ __forceinline__ double* blkS(int gr, int gc) const { return p.S + (size_t)gr * BLK * p.m + (size_t)gc * BLK; }
+    // TMA coordinates {inner element, row} of block (gr, gc) in the [tiles*t, t] view of L / V^T
+    __device__ __forceinline__ int2 crdL(int gr, int gc) const {
+        const int I = gr / p.nbt, J = gc / p.nbt;
+        return make_int2((gc % p.nbt) * BLK, (I * (I + 1) / 2 + J) * p.t + (gr % p.nbt) * BLK);
+    }
+    __device__ __forceinline__ int2 crdV(int gr, int gc) const {
+        const int I = gr / p.nbt, J = gc / p.nbt;
+        return make_int2((gc % p.nbt) * BLK, (I * p.Mt + J) * p.t + (gr % p.nbt) * BLK);
+    }
+    // number of writes after which block (gr,gc) of L is final
+    __device__ __forceinline__ int finL(int gr, int gc) const {
+        const int K = gc / p.nbt, bk = gc % p.nbt;
+        return (gr / p.nbt == K) ? K + 1 + bk : K + 1 + (bk > 0 ? 1 : 0);
+    }
+    __device__ __forceinline__ int finV(int gc) const { return gc / p.nbt + 1 + (gc % p.nbt > 0 ? 1 : 0); }
+
+    // ---- dependency polling: wait w of the current job is handled by lane w % 32 ------------------
+    __device__ __forceinline__ void poll(const int* addr, int need) {
+        if (addr != nullptr && need > 0) {
+            const int target = need * kConsumerWarps;
+            unsigned spins = 0;
+            (void)spins;
+            while (ld_acquire(addr) < target) {
+                GPB_SPIN_GUARD(spins, "dependency poll", target, ld_acquire(addr))
+                __nanosleep(40);
+            }
+        }
+    }
+    __device__ __forceinline__ void deps_done(long long t0) {
+        __syncwarp();
+        fence_proxy_async_global();      // acquired generic-proxy writes -> visible to the TMA reads issued below
+        if (lane == 0) poll_cycles += clock64() - t0;
+    }
+
+    // ---- job hand-off and operand streaming ------------------------------------------------------
+    // Lane 0 alone runs the mbarrier / TMA protocol (its stage, phase, slot, jphase are the only live
+    // copies); the other lanes help with dependency polling and L2 prefetch and meet lane 0 again at
+    // the __syncwarp() of the next job's deps_done().
+    __device__ __forceinline__ void push_job(double* C, int* sig, int ldc, int nk, int kind, int arg) {
+        if (lane != 0) return;
+        mbar_wait(&job_empty[slot], (uint32_t)(jphase ^ 1), 1);
+        Job j;
+        j.C = C; j.sig = sig; j.ldc = ldc; j.nk = nk; j.kind = kind; j.arg = arg;
+        jobs[slot] = j;
+        mbar_arrive(&job_full[slot]);
+        if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
+    }
+    __device__ __forceinline__ void stream(const CUtensorMap* mA, int2 a, const CUtensorMap* mB, int2 b, int nk) {
+        if (lane != 0) return;
+        for (int kt = 0; kt < nk; ++kt) {
+            mbar_wait(&empty[stage], (uint32_t)(phase ^ 1), 2);
+            char* dst = ring + (size_t)stage * Cfg::kStageBytes;
+            mbar_arrive_expect_tx(&full[stage], (uint32_t)Cfg::kStageBytes);
+            tma_load_2d(dst, mA, a.x + kt * kBK, a.y, &full[stage]);
+            tma_load_2d(dst + Cfg::kOperandBytes, mB, b.x + kt * kBK, b.y, &full[stage]);
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+    }
+    // warm L2 with the rows of the C block the consumers will read in their epilogue
+    __device__ __forceinline__ void prefetch_c(const double* C, int ldc) {
+        for (int r = lane; r < BLK; r += 32) l2_prefetch_bulk(C + (size_t)r * ldc, BLK * 8);
+    }
+
+    // C(gr,gc) -= A(gr,q0:q1) B(gc,q0:q1)^T on (matC, matA, matB) given by op
+    __device__ void update(uint32_t op, int gr, int gc, int q0, int q1) {
+        const int nq = q1 - q0;
+        const long long t0 = clock64();
+        if (!p.no_deps) {
+            // waits: 0: own block; 1..nq: A panel; 1+nq..2nq: B panel
+            for (int w = lane; w < 1 + 2 * nq; w += 32) {
+                const int* addr = nullptr;
+                int need = 0;
+                if (op == OP_UPD_L) {
+                    if (w == 0) { addr = p.verL + (size_t)gr * p.NB + gc; need = q0 / p.nbt + q0 % p.nbt; }
+                    else if (w <= nq) { const int q = q0 + w - 1; addr = p.verL + (size_t)gr * p.NB + q; need = finL(gr, q); }
+                    else { const int q = q0 + w - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
+                } else if (op == OP_UPD_V) {
+                    if (w == 0) { addr = p.verV + (size_t)gr * p.NB + gc; need = q0 / p.nbt; }
+                    else if (w <= nq) { const int q = q0 + w - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
+                    else if (!p.L_final) { const int q = q0 + w - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
+                } else {  // OP_UPD_S
+                    if (w == 0) { addr = p.verS + (size_t)gr * p.NBm + gc; need = q0 / p.nbt; }
+                    else if (w <= nq) { const int q = q0 + w - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
+                    else { const int q = q0 + w - 1 - nq; addr = p.verV + (size_t)gc * p.NB + q; need = finV(q); }
+                }
+                poll(addr, need);
+            }
+        }
+        deps_done(t0);
+        const int nk = nq * BLK / kBK;
+        if (op == OP_UPD_L) {
+            double* C = blkL(gr, gc);
+            prefetch_c(C, p.t);
+            push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
+            stream(mapL, crdL(gr, q0), mapL, crdL(gc, q0), nk);
+        } else if (op == OP_UPD_V) {
+            double* C = blkV(gr, gc);
+            prefetch_c(C, p.t);
+            push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
+            stream(mapV, crdV(gr, q0), mapL, crdL(gc, q0), nk);
+        } else {
+            double* C = blkS(gr, gc);
+            prefetch_c(C, (int)p.m);
+            push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, 0);
+            stream(mapV, crdV(gr, q0), mapV, crdV(gc, q0), nk);
+        }
+    }
+
+    // C(gr,gc) = C(gr,gc) invD(gc)^T   (is_v: C is a block of V^T, else of L)
+    __device__ void trsm(bool is_v, int gr, int gc) {
+        const long long t0 = clock64();
+        if (!p.no_deps) {
+            if (lane == 0) {
+                if (is_v) poll(p.verV + (size_t)gr * p.NB + gc, finV(gc) - 1);
+                else poll(p.verL + (size_t)gr * p.NB + gc, finL(gr, gc) - 1);
+            } else if (lane == 1 && !(is_v && p.L_final)) {
+                poll(p.verL + (size_t)gc * p.NB + gc, finL(gc, gc));
+            }
+        }
+        deps_done(t0);
+        const int2 d = make_int2(0, gc * BLK);
+        if (is_v) {
+            push_job(blkV(gr, gc), p.verV + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 0);
+            stream(mapV, crdV(gr, gc), mapD, d, BLK / kBK);
+        } else {
+            push_job(blkL(gr, gc), p.verL + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 0);
+            stream(mapL, crdL(gr, gc), mapD, d, BLK / kBK);
+        }
+    }
+
+    __device__ void row_chain(bool is_v, int gr, int qt) {
+        for (int jj = 0; jj < p.nbt; ++jj) {
+            if (jj > 0) update(is_v ? OP_UPD_V : OP_UPD_L, gr, qt + jj, qt, qt + jj);
+            trsm(is_v, gr, qt + jj);
+        }
+    }
+
+    // The consumers factor the block inside the operand ring: no TMA may be in flight into it, so
+    // the producer hands the job over and then waits for the block's final version before it streams again.
+    __device__ void potrf(int q) {
+        const long long t0 = clock64();
+        int* ver = p.verL + (size_t)q * p.NB + q;
+        if (lane == 0 && !p.no_deps) poll(ver, finL(q, q) - 1);
+        deps_done(t0);
+        push_job(blkL(q, q), ver, p.t, 0, JOB_POTRF, q);
+        const long long t1 = clock64();
+        if (lane == 0) poll(ver, finL(q, q));
+        __syncwarp();
+        if (lane == 0) poll_cycles += clock64() - t1;
+    }
+
+    __device__ void run(const Item& it) {
+        switch (it.op) {
+            case OP_UPD_L: case OP_UPD_V: case OP_UPD_S:
+                update(it.op, (int)it.gr, (int)it.gc, (int)(it.q & 0xffffu), (int)(it.q >> 16)); break;
+            case OP_TRSM_L: trsm(false, (int)it.gr, (int)it.gc); break;
+            case OP_POTRF: potrf((int)it.gc); break;
+            case OP_ROW_L: row_chain(false, (int)it.gr, (int)it.gc); break;
+            case OP_ROW_V: row_chain(true, (int)it.gr, (int)it.gc); break;
+            default: break;
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// The consumer warps.
+// ---------------------------------------------------------------------------------------------
+template <int BLK>
+__device__ void consumer_loop(const ExecParams& p, char* base) {
+    using Cfg = GemmCfg<BLK>;
+    using SM = ExecSmem<BLK>;
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + SM::kFull);
+    uint64_t* empty = reinterpret_cast<uint64_t*>(base + SM::kEmpty);
+    uint64_t* job_full = reinterpret_cast<uint64_t*>(base + SM::kJobFull);
+    uint64_t* job_empty = reinterpret_cast<uint64_t*>(base + SM::kJobEmpty);
+    const Job* jobs = reinterpret_cast<const Job*>(base + SM::kJobs);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    WarpTile<BLK> w;
+    w.init(warp, lane);
+    int stage = 0, phase = 0, slot = 0, jphase = 0;
+    int pending = -1;                      // ring stage consumed but not yet released
+    for (;;) {
+        mbar_wait(&job_full[slot], (uint32_t)jphase, 3);
+        const Job j = jobs[slot];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&job_empty[slot]);
+        if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
+        if (j.kind == JOB_EXIT) break;
+        if (j.kind == JOB_POTRF) {
+            // every earlier stage has been consumed by this warp; the barrier inside makes that true for all warps
+            cbar();
+            potrf_block<BLK>(reinterpret_cast<double*>(base), j.C, j.ldc, p.invD + (size_t)j.arg * BLK * BLK, p.d_info, j.arg * BLK);
+            fence_proxy_async_global();      // L(q,q), invD(q): read by other CTAs' TMA
+            fence_proxy_async_shared();      // the ring is about to be overwritten by TMA again
+            __threadfence();
+            cbar();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                atomicAdd(j.sig, kConsumerWarps);
+            }
+            continue;
+        }
+        double acc[Cfg::MI][Cfg::NJ][2];
+#pragma unroll
+        for (int i = 0; i < Cfg::MI; ++i)
+#pragma unroll
+            for (int jj = 0; jj < Cfg::NJ; ++jj) acc[i][jj][0] = acc[i][jj][1] = 0.0;
+        for (int kt = 0; kt < j.nk; ++kt) {
+            mbar_wait(&full[stage], (uint32_t)phase, 4);
+            // Deferred release: the stage consumed one step ago is handed back only now.  Releasing a
+            // stage right behind its last LDS.64 is NOT safe -- the arrive does not wait for loads
+            // still in flight and the TMA refill then races them (measured: 11 of 80 runs of config 2
+            // came out wrong at 1e-5; 0 of 80 with either a fence.acq_rel.cta before the arrive or
+            // this deferral, which costs nothing but one stage of ring depth).  By now every DMMA of
+            // the previous stage has issued, so every load of it has returned.  `pending` carries
+            // across jobs; a stage still pending at a POTRF or at EXIT is simply not needed.
+            if (pending >= 0) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[pending]);
+            }
+            pending = stage;
+            consume_stage<BLK>(base + (size_t)stage * Cfg::kStageBytes, w, acc);
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+        store_tile<BLK>(j.C, j.ldc, j.kind, w, acc);
+        fence_proxy_async_global();          // this warp's part of C: read by TMA later
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence();
+            atomicAdd(j.sig, 1);
+        }
+    }
 }
 
 // The persistent executor kernel.
 template <int BLK>
-__global__ void __launch_bounds__(kThreads, 1) exec_kernel(const __grid_constant__ ExecParams p) {
-    extern __shared__ __align__(16) double smem[];
-    __shared__ unsigned int s_ticket;
-    __shared__ long long s_wait;
-    if (threadIdx.x == 0) s_wait = 0;
+__global__ void __launch_bounds__(kThreads, 1)
+exec_kernel(const __grid_constant__ ExecParams p, const __grid_constant__ CUtensorMap mapL, const __grid_constant__ CUtensorMap mapV,
+            const __grid_constant__ CUtensorMap mapD) {
+    extern __shared__ char smem_raw[];
+    using SM = ExecSmem<BLK>;
+    char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        uint64_t* full = reinterpret_cast<uint64_t*>(base + SM::kFull);
+        uint64_t* empty = reinterpret_cast<uint64_t*>(base + SM::kEmpty);
+        uint64_t* job_full = reinterpret_cast<uint64_t*>(base + SM::kJobFull);
+        uint64_t* job_empty = reinterpret_cast<uint64_t*>(base + SM::kJobEmpty);
+        for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kConsumerWarps); }
+        for (int s = 0; s < kJobSlots; ++s) { mbar_init(&job_full[s], 1); mbar_init(&job_empty[s], kConsumerWarps); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    if (warp < kConsumerWarps) {
+        reg_alloc<kConsumerRegs>();
+        consumer_loop<BLK>(p, base);
+        return;
+    }
+    reg_dealloc<kProducerRegs>();
+    if (warp != kConsumerWarps) return;     // the rest of the producer warpgroup only gives its registers away
+    // ---- producer warp ----
     const long long t_start = clock64();
+    if (lane == 0) { tma_prefetch_desc(&mapL); tma_prefetch_desc(&mapV); tma_prefetch_desc(&mapD); }
+    Producer<BLK> prod(p, &mapL, &mapV, &mapD, base);
     unsigned long long nrun = 0;
-    Exec<BLK> ex(p, smem, &s_wait);
     for (;;) {
-        if (threadIdx.x == 0) s_ticket = atomicAdd(p.ticket, 1u);
-        __syncthreads();
-        const unsigned int tk = s_ticket;
+        unsigned int tk = 0;
+        if (lane == 0) tk = atomicAdd(p.ticket, 1u);
+        tk = __shfl_sync(0xffffffffu, tk, 0);
         if (tk >= (unsigned int)p.nitems) break;
         const int4 raw = __ldg(reinterpret_cast<const int4*>(p.items) + tk);
         Item it;
         it.op = (uint32_t)raw.x; it.gr = (uint32_t)raw.y; it.gc = (uint32_t)raw.z; it.q = (uint32_t)raw.w;
-        ex.run(it);
+        prod.run(it);
         ++nrun;
-        // run() always ends with signal(), whose barrier also protects s_ticket and the ring
     }
-    if (threadIdx.x == 0 && p.stats != nullptr) {
+    prod.push_job(nullptr, nullptr, 0, 0, JOB_EXIT, 0);
+    if (lane == 0 && p.stats != nullptr) {
         unsigned int smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         unsigned long long* st = p.stats + 4 * (size_t)blockIdx.x;
-        st[0] = (unsigned long long)s_wait;
+        st[0] = (unsigned long long)prod.poll_cycles;
         st[1] = (unsigned long long)(clock64() - t_start);
         st[2] = nrun;
         st[3] = smid;
@@ -305,10 +505,10 @@ __global__ void __launch_bounds__(kThreads, 1) exec_kernel(const __grid_constant
 }
 
 // Batched inverse of the diagonal blocks of L (used by gp_solve and gp_predict_full_cov, which
-// receive only L): one CTA per diagonal block.
+// receive only L): one CTA of kConsumerThreads per diagonal block.
 template <int BLK>
-__global__ void __launch_bounds__(kThreads, 1) trtri_diag_kernel(const double* __restrict__ L, int t, int nbt,
-                                                                  double* __restrict__ invD) {
+__global__ void __launch_bounds__(kConsumerThreads, 1) trtri_diag_kernel(const double* __restrict__ L, int t, int nbt,
+                                                                          double* __restrict__ invD) {
     extern __shared__ __align__(16) double smem[];
     constexpr int SP = BLK + 1;
     const int q = blockIdx.x;
@@ -317,15 +517,10 @@ __global__ void __launch_bounds__(kThreads, 1) trtri_diag_kernel(const double* _
     load_lower_to_smem<BLK>(smem, G, t);
     inv_lower_smem<BLK>(smem);
     double* inv = invD + (size_t)q * BLK * BLK;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kThreads) {
+    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
         const int r = idx / BLK, c = idx % BLK;
         inv[idx] = smem[r * SP + c];
     }
-}
-
-template <int BLK>
-constexpr int exec_smem_bytes() {
-    return GemmCfg<BLK>::kSmemBytes > BLK * (BLK + 1) * 8 ? GemmCfg<BLK>::kSmemBytes : BLK * (BLK + 1) * 8;
 }
 
 }  // namespace gpb

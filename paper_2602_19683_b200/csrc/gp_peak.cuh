@@ -51,4 +51,5 @@ __global__ void __launch_bounds__(kPeakThreads) peak_dfma_kernel(double* __restr
     if (s == 123.456) sink[0] = s;
 }
 
+
 }  // namespace gpb

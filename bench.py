@@ -39,7 +39,7 @@ METRIC = "FP64 tiled Cholesky GFLOP/s and full-cov prediction time at n=32768; %
 # DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant
 # kernel (exec_kernel<128>, the Cholesky DAG) from the ncu --set full capture summarised in
 # profiles/; keyed by (n, tile).  None = not captured for this workload.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {(32768, 1024): 572.2e9}   # profiles/r01b_ncu_exec_kernel_cholesky_c3.md
 
 ORACLE_SAMPLE_BASELINE = (4096, 512)    # (n, m) of the cpu_baseline leg: ~10-30 s of CPU work
 ORACLE_SAMPLE_REFERENCE = (3072, 384)   # per step of --impl reference
@@ -241,6 +241,15 @@ def measure_fp64_peak(gp, torch):
                 gp.gp_fp64_peak_launch(mode, iters, sink)
             b.record(); torch.cuda.synchronize()
             out["dmma_sustained_tflops"] = reps * flops / (a.elapsed_time(b) * 1e-3) / 1e12
+    # the contraction path alone (TMA stream + DMMA loop + epilogue + signalling, no DAG): K = 1024 items
+    K, reps = 1024, 100
+    buf = (torch.rand(gp.gp_contraction_bench_bytes(K, reps) // 8 + 1, dtype=torch.float64, device="cuda") * 1e-3).view(torch.uint8)
+    for _ in range(2):
+        flops = gp.gp_contraction_bench_launch(K, reps, buf)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); flops = gp.gp_contraction_bench_launch(K, reps, buf); b.record(); torch.cuda.synchronize()
+    out["contraction_k1024_tflops"] = flops / (a.elapsed_time(b) * 1e-3) / 1e12
     return out
 
 
@@ -348,12 +357,14 @@ def run_b200(args):
                     "ms": e2e_ms, "h2d_bytes_per_step": (n * D + n + m * D) * 8, "d2h_bytes_per_step": (m + m * m) * 8 + 4,
                     "info": info_e2e, "call": "gp_pipeline_host (pinned host buffers)"},
             "gpu_launches": sum(LAUNCHES_PER_STEP.values()) * args.steps,
-            "roofline": {"bound": "tensor", "kernel": "exec_kernel<128> (tiled Cholesky DAG: POTRF/TRSM/SYRK/GEMM, FP64 DMMA)",
+            "roofline": {"bound": "tensor", "kernel": "exec_kernel<128> (tiled Cholesky DAG: POTRF/TRSM/SYRK/GEMM; TMA-fed FP64 DMMA)",
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                          "peak_source": "gp_fp64_peak_launch DMMA.8x8x4 register-resident microbenchmark, measured live, "
                                         "sustained ~2 s loop (kernel is timed inside a long step)",
                          "peak_burst": peaks["dmma_burst_tflops"], "dfma_burst": peaks["dfma_burst_tflops"],
                          "frac_of_burst": achieved / peaks["dmma_burst_tflops"],
+                         "contraction_alone_tflops": peaks["contraction_k1024_tflops"],
+                         "full_cov_exec_tflops": (n * n * m + n * m * m) / (phase["full_cov"] * 1e-3) / 1e12,
                          "hbm_gbs_measured": mp.get("hbm_gbs"),
                          "assemble_gbs": (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["assemble"] * 1e-3) / 1e9,
                          "solve_gbs": 2 * (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["solve"] * 1e-3) / 1e9},

@@ -162,9 +162,13 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
 
 /* Executor statistics of the LAST gp_cholesky_tiled / gp_predict_full_cov call that used dWork
  * (tracing support; the analogue of the paper's per-step APEX timers).  Copies
- * to h_stats (host) 4 uint64 per worker CTA: {SM cycles spent waiting on dependencies, SM cycles
- * from kernel start to the worker's exit, work items run, SM id}; synchronises the stream.
- * Returns the number of worker slots copied (<= max_workers) or a negative GP_ERR_*. */
+ * to h_stats (host) 8 uint64 per worker CTA:
+ *   [0] SM cycles its producer warp spent polling dependency counters,
+ *   [1] SM cycles from kernel start to the producer's exit,  [2] work items run,  [3] SM id,
+ *   [4] SM cycles consumer warp 0 waited for a job descriptor (nothing runnable was handed over),
+ *   [5] reserved,  [6] jobs (GEMM / POTRF block operations) run,  [7] reserved;
+ * synchronises the stream.  Returns the number of worker slots copied (<= max_workers) or a
+ * negative GP_ERR_*. */
 int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream);
 
 /* Host-only self-check of the static work-item schedule the persistent executor consumes (a6):

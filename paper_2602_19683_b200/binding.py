@@ -223,12 +223,13 @@ def gp_schedule_selfcheck(n: int, m: int, tile: int, workers: int = 148):
 
 
 def gp_exec_stats(work: torch.Tensor, max_workers: int = 148):
-    """Per-worker (wait_cycles, total_cycles, items, sm_id) of the last executor launch that used `work`."""
-    buf = (ctypes.c_uint64 * (4 * max_workers))()
+    """Per-worker (producer_poll_cycles, total_cycles, items, sm_id, consumer_job_wait_cycles,
+    0, jobs, 0) of the last executor launch that used `work`."""
+    buf = (ctypes.c_uint64 * (8 * max_workers))()
     w = int(load().gp_exec_stats(_ptr(work, torch.uint8), buf, max_workers, _stream()))
     if w < 0:
         raise GpError(w, "gp_exec_stats")
-    return [tuple(buf[4 * i:4 * i + 4]) for i in range(w)]
+    return [tuple(buf[8 * i:8 * i + 8]) for i in range(w)]
 
 
 def gp_release_cached_schedules() -> None:

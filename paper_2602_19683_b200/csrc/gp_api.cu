@@ -24,8 +24,9 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // workspace common header: [0, 256) ticket counters, [256, kHdrBytes) per-worker executor statistics
 constexpr size_t kStatsOff = 256;
-constexpr size_t kHdrBytes = 8192;
-constexpr int kMaxWorkers = (int)((kHdrBytes - kStatsOff) / 32);
+constexpr size_t kHdrBytes = 16384;
+constexpr size_t kStatsBytes = 64;   // 8 uint64 per worker, see gp_exec_stats
+constexpr int kMaxWorkers = (int)((kHdrBytes - kStatsOff) / kStatsBytes);
 
 int pick_block(int tile) {
     if (tile % 128 == 0) return 128;
@@ -607,7 +608,7 @@ extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_worke
     if (max_workers <= 0) return GP_ERR_SIZE;
     const int w = max_workers < kMaxWorkers ? max_workers : kMaxWorkers;
     cudaStream_t st = (cudaStream_t)stream;
-    if (cudaMemcpyAsync(h_stats, (const char*)dWork + kStatsOff, (size_t)w * 32, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpyAsync(h_stats, (const char*)dWork + kStatsOff, (size_t)w * kStatsBytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
     return cudaStreamSynchronize(st) == cudaSuccess ? w : GP_ERR_CUDA;
 }
 

@@ -70,7 +70,7 @@ struct ExecParams {
     int64_t m;             // rows of Sigma (leading dimension)
     int L_final;           // 1: L is an input that is final everywhere (predictor), no waits on it
     int no_deps;           // 1: skip every dependency wait (contraction microbenchmark only)
-    unsigned long long* stats;   // per worker CTA: {producer cycles polling dependencies, cycles total, items run, SM id}
+    unsigned long long* stats;   // 8 per worker CTA, see gp_exec_stats in include/gp_b200.h
 };
 
 enum JobKind : int { JOB_GEMM_SUB = 0, JOB_GEMM_SET = 1, JOB_POTRF = 2, JOB_EXIT = 3 };
@@ -396,13 +396,19 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
     w.init(warp, lane);
     int stage = 0, phase = 0, slot = 0, jphase = 0;
     int pending = -1;                      // ring stage consumed but not yet released
+    const bool keeper = (threadIdx.x == 0) && p.stats != nullptr;     // consumer-side statistics
+    long long job_wait = 0;
+    unsigned int njobs = 0;
     for (;;) {
+        const long long tj = clock64();
         mbar_wait(&job_full[slot], (uint32_t)jphase, 3);
+        if (keeper) job_wait += clock64() - tj;
         const Job j = jobs[slot];
         __syncwarp();
         if (lane == 0) mbar_arrive(&job_empty[slot]);
         if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
         if (j.kind == JOB_EXIT) break;
+        ++njobs;
         if (j.kind == JOB_POTRF) {
             // every earlier stage has been consumed by this warp; the barrier inside makes that true for all warps
             cbar();
@@ -447,6 +453,12 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
             __threadfence();
             atomicAdd(j.sig, 1);
         }
+    }
+    if (keeper) {
+        unsigned long long* st = p.stats + 8 * (size_t)blockIdx.x;
+        st[4] = (unsigned long long)job_wait;
+        st[5] = 0;
+        st[6] = (unsigned long long)njobs;
     }
 }
 
@@ -496,7 +508,7 @@ exec_kernel(const __grid_constant__ ExecParams p, const __grid_constant__ CUtens
     if (lane == 0 && p.stats != nullptr) {
         unsigned int smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        unsigned long long* st = p.stats + 4 * (size_t)blockIdx.x;
+        unsigned long long* st = p.stats + 8 * (size_t)blockIdx.x;
         st[0] = (unsigned long long)prod.poll_cycles;
         st[1] = (unsigned long long)(clock64() - t_start);
         st[2] = nrun;

@@ -85,7 +85,7 @@ void item_effects(const Shape& s, const SchedItem& it, FW&& wait, FR&& write) {
 struct Cost {
     double per_q, fixed, potrf;
     explicit Cost(int blk) {
-        if (blk >= 128) { per_q = 19.5; fixed = 4.0; potrf = 45.0; }
+        if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 45.0; }
         else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 14.0; }
         else { per_q = 0.8; fixed = 2.5; potrf = 6.0; }
     }
@@ -111,42 +111,63 @@ inline SchedItem mk(uint32_t op, int gr, int gc, int q0 = 0, int q1 = 0) {
     return it;
 }
 
-void program_order_cholesky(int M, int nbt, std::vector<SchedItem>& v) {
+// `task` receives, per item, the index of the paper's tile task it belongs to:
+// the scheduler keeps the block items of one tile task together so that they share operand panels in L2.
+void program_order_cholesky(int M, int nbt, std::vector<SchedItem>& v, std::vector<int32_t>& task) {
+    int32_t tid = 0;
+    auto emit = [&](const SchedItem& it) { v.push_back(it); task.push_back(tid); };
     for (int J = 0; J < M; ++J) {
         const int qt = J * nbt;
-        // POTRF tile task = right-looking block Cholesky of the diagonal tile
+        // POTRF tile task = right-looking block Cholesky of the diagonal tile; its items are
+        // on the critical path and are scheduled one by one
         for (int jj = 0; jj < nbt; ++jj) {
-            v.push_back(mk(S_POTRF, qt + jj, qt + jj));
-            for (int ii = jj + 1; ii < nbt; ++ii) v.push_back(mk(S_TRSM_L, qt + ii, qt + jj));
+            emit(mk(S_POTRF, qt + jj, qt + jj)); ++tid;
+            for (int ii = jj + 1; ii < nbt; ++ii) { emit(mk(S_TRSM_L, qt + ii, qt + jj)); ++tid; }
             for (int kk = jj + 1; kk < nbt; ++kk)
-                for (int ii = kk; ii < nbt; ++ii) v.push_back(mk(S_UPD_L, qt + ii, qt + kk, qt + jj, qt + jj + 1));
+                for (int ii = kk; ii < nbt; ++ii) { emit(mk(S_UPD_L, qt + ii, qt + kk, qt + jj, qt + jj + 1)); ++tid; }
         }
         // TRSM tile tasks: one chain per block row
-        for (int I = J + 1; I < M; ++I)
-            for (int bi = 0; bi < nbt; ++bi) v.push_back(mk(S_ROW_L, I * nbt + bi, qt));
+        for (int I = J + 1; I < M; ++I) {
+            for (int bi = 0; bi < nbt; ++bi) emit(mk(S_ROW_L, I * nbt + bi, qt));
+            ++tid;
+        }
         // SYRK and GEMM tile tasks
         for (int K = J + 1; K < M; ++K)
-            for (int I = K; I < M; ++I)
+            for (int I = K; I < M; ++I) {
                 for (int bk = 0; bk < nbt; ++bk)
                     for (int bi = (I == K ? bk : 0); bi < nbt; ++bi)
-                        v.push_back(mk(S_UPD_L, I * nbt + bi, K * nbt + bk, qt, qt + nbt));
+                        emit(mk(S_UPD_L, I * nbt + bi, K * nbt + bk, qt, qt + nbt));
+                ++tid;
+            }
     }
 }
 
-void program_order_predict(int M, int Mm, int nbt, std::vector<SchedItem>& v) {
+void program_order_predict(int M, int Mm, int nbt, std::vector<SchedItem>& v, std::vector<int32_t>& task) {
+    int32_t tid = 0;
+    auto emit = [&](const SchedItem& it) { v.push_back(it); task.push_back(tid); };
     for (int J = 0; J < M; ++J) {
         const int qt = J * nbt;
-        for (int a = 0; a < Mm * nbt; ++a) v.push_back(mk(S_ROW_V, a, qt));                      // V^T_{a,J} = (..) L_JJ^-T
-        for (int P = J + 1; P < M; ++P)                                                           // V^T_{a,P} -= V^T_{a,J} L_{P,J}^T
-            for (int bk = 0; bk < nbt; ++bk)
-                for (int a = 0; a < Mm * nbt; ++a) v.push_back(mk(S_UPD_V, a, P * nbt + bk, qt, qt + nbt));
-        for (int b = 0; b < Mm * nbt; ++b)                                                        // Sigma_{a,b} -= V^T_{a,J} V^T_{b,J}^T
-            for (int a = b; a < Mm * nbt; ++a) v.push_back(mk(S_UPD_S, a, b, qt, qt + nbt));
+        for (int A = 0; A < Mm; ++A) {                                                            // V^T_{A,J} = (..) L_JJ^-T
+            for (int ba = 0; ba < nbt; ++ba) emit(mk(S_ROW_V, A * nbt + ba, qt));
+            ++tid;
+        }
+        for (int P = J + 1; P < M; ++P)                                                           // V^T_{A,P} -= V^T_{A,J} L_{P,J}^T
+            for (int A = 0; A < Mm; ++A) {
+                for (int bk = 0; bk < nbt; ++bk)
+                    for (int ba = 0; ba < nbt; ++ba) emit(mk(S_UPD_V, A * nbt + ba, P * nbt + bk, qt, qt + nbt));
+                ++tid;
+            }
+        for (int B = 0; B < Mm; ++B)                                                              // Sigma_{A,B} -= V^T_{A,J} V^T_{B,J}^T
+            for (int A = B; A < Mm; ++A) {
+                for (int bb = 0; bb < nbt; ++bb)
+                    for (int ba = (A == B ? bb : 0); ba < nbt; ++ba) emit(mk(S_UPD_S, A * nbt + ba, B * nbt + bb, qt, qt + nbt));
+                ++tid;
+            }
     }
 }
 
-void schedule(const Shape& s, std::vector<SchedItem>& prog, int workers, int blk, std::vector<SchedItem>& out,
-              SchedStats* stats, bool simulate) {
+void schedule(const Shape& s, std::vector<SchedItem>& prog, const std::vector<int32_t>& task, int workers, int blk,
+              std::vector<SchedItem>& out, SchedStats* stats, bool simulate) {
     const int N = (int)prog.size();
     if (!simulate || N == 0) { out = prog; return; }
     const Cost cost(blk);
@@ -198,13 +219,24 @@ void schedule(const Shape& s, std::vector<SchedItem>& prog, int workers, int blk
         for (int i = 0; i < N; ++i)
             for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) sucs[fill[deps[e]]++] = i;
     }
-    // 4. list scheduling
+    // 4. list scheduling.  Priority = the critical-path length of the item's TILE TASK (the maximum over
+    // its block items), ties by program order: ready items of one tile task leave the queue together,
+    // so the ~148 items in flight belong to two or three tile tasks and share their operand panels in L2
+    // (ordering single items by their own bottom level interleaves dozens of tile tasks: 572 GB of DRAM
+    // traffic per factorisation at n = 32768 instead of ~150 GB, profiles/r01b).
+    std::vector<float> prio(N);
+    {
+        const int32_t ntask = N > 0 ? task[N - 1] + 1 : 0;
+        std::vector<float> tmax(ntask, 0.f);
+        for (int i = 0; i < N; ++i) tmax[task[i]] = std::max(tmax[task[i]], bottom[i]);
+        for (int i = 0; i < N; ++i) prio[i] = tmax[task[i]];
+    }
     std::vector<int32_t> missing(N);
-    using PR = std::pair<float, int32_t>;                       // (bottom level, -item) max-heap
+    using PR = std::pair<float, int32_t>;                       // (task priority, -item) max-heap
     std::priority_queue<PR> ready;
     for (int i = 0; i < N; ++i) {
         missing[i] = (int32_t)(dep_off[i + 1] - dep_off[i]);
-        if (missing[i] == 0) ready.push(PR(bottom[i], -i));
+        if (missing[i] == 0) ready.push(PR(prio[i], -i));
     }
     using EV = std::pair<double, int32_t>;                      // (finish time, item) min-heap
     std::priority_queue<EV, std::vector<EV>, std::greater<EV>> running;
@@ -229,7 +261,7 @@ void schedule(const Shape& s, std::vector<SchedItem>& prog, int workers, int blk
             ++idle;
             for (int64_t e = suc_off[i]; e < suc_off[i + 1]; ++e) {
                 const int sc = sucs[e];
-                if (--missing[sc] == 0) ready.push(PR(bottom[sc], -sc));
+                if (--missing[sc] == 0) ready.push(PR(prio[sc], -sc));
             }
         }
         makespan = now;
@@ -249,14 +281,16 @@ void schedule(const Shape& s, std::vector<SchedItem>& prog, int workers, int blk
 
 void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate) {
     std::vector<SchedItem> prog;
-    program_order_cholesky(M, nbt, prog);
-    schedule(Shape(M, 0, nbt, false), prog, workers, blk, out, stats, simulate);
+    std::vector<int32_t> task;
+    program_order_cholesky(M, nbt, prog, task);
+    schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, stats, simulate);
 }
 
 void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate) {
     std::vector<SchedItem> prog;
-    program_order_predict(M, Mm, nbt, prog);
-    schedule(Shape(M, Mm, nbt, true), prog, workers, blk, out, stats, simulate);
+    std::vector<int32_t> task;
+    program_order_predict(M, Mm, nbt, prog, task);
+    schedule(Shape(M, Mm, nbt, true), prog, task, workers, blk, out, stats, simulate);
 }
 
 bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why) {
@@ -283,7 +317,8 @@ bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int n
         }
     }
     std::vector<SchedItem> prog;
-    if (predict) program_order_predict(M, Mm, nbt, prog); else program_order_cholesky(M, nbt, prog);
+    std::vector<int32_t> task;
+    if (predict) program_order_predict(M, Mm, nbt, prog, task); else program_order_cholesky(M, nbt, prog, task);
     if (prog.size() != items.size()) { if (why) *why = kCount; return false; }
     return true;
 }

@@ -183,6 +183,21 @@ int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaSt
     }
 }
 
+template <int SB>
+int launch_solves(const double* dL, int tile, int NB, const double* invD, const double* dY, double* beta, double* dAlpha, int* flags,
+                  unsigned int* ticket, cudaStream_t st) {
+    static bool configured = false;
+    constexpr int smem = SolveCfg<SB>::kSmemBytes;
+    if (!configured) {
+        if (cudaFuncSetAttribute(forward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
+        if (cudaFuncSetAttribute(backward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
+        configured = true;
+    }
+    forward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
+    backward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
 int workers_for(int sched_width) {
     const int sms = sm_count();
     if (sched_width <= 0) return sms < kMaxWorkers ? sms : kMaxWorkers;
@@ -367,19 +382,11 @@ int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dA
     rc = launch_trtri_any(b, dL, tile, NB, invD, st);
     if (rc != GP_OK) return rc;
     switch (b) {
-        case 128:
-            forward_solve_kernel<128><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
-            backward_solve_kernel<128><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
-            break;
-        case 64:
-            forward_solve_kernel<64><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
-            backward_solve_kernel<64><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
-            break;
-        default:
-            forward_solve_kernel<32><<<NB, 256, 0, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
-            backward_solve_kernel<32><<<NB, 256, 0, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
-            break;
+        case 128: rc = launch_solves<128>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
+        case 64: rc = launch_solves<64>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
+        default: rc = launch_solves<32>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
     }
+    if (rc != GP_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 

@@ -132,89 +132,117 @@ __global__ void mirror_lower_kernel(double* __restrict__ S, int64_t m) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Triangular solves for alpha.  Block rows/columns of 128 (kSB) regardless of the
-// tile size (tile % 32 == 0 is handled by kSB = gcd-style choice made on the host: sb divides
-// tile).  One CTA per block row; rows are handed out by a ticket so that a CTA only ever waits
-// for rows claimed before it.  The off-diagonal part is a streaming GEMV that consumes x_p as
-// soon as block p publishes it; the diagonal block is applied as a GEMV with its inverse.
+// Triangular solves for alpha.  Block rows/columns of SB (= the executor's block
+// edge).  One CTA per block row; rows are handed out by a ticket so that a CTA only ever waits for
+// rows claimed before it.  The off-diagonal part is a streaming GEMV that consumes x_p as soon as
+// block p publishes it; the diagonal block is applied as a GEMV with its inverse.
+//
+// The n/SB diagonal steps form a latency chain (x_i needs x_{i-1}); everything else is bandwidth.
+// To keep the chain short, a CTA (a) copies its inverted diagonal block into shared memory with
+// cp.async before it starts streaming, (b) loads every block of L into registers BEFORE it waits
+// for the matching piece of x, so that on the critical last block only the flag, 4 doubles of x,
+// two shuffle reductions and the publish remain, and (c) lets every warp poll the flag itself
+// instead of going through a CTA barrier.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int ld_acquire_i(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void cp_async16_solve(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all_solve() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
 __device__ __forceinline__ const double* tile_block_ptr(const double* L, int t, int sbt, int gr, int gc, int sb) {
     const int I = gr / sbt, J = gc / sbt;
     return L + ((size_t)I * (I + 1) / 2 + J) * (size_t)t * t + (size_t)(gr % sbt) * sb * t + (size_t)(gc % sbt) * sb;
 }
 
-// Forward: x_i = invD_i (y_i - sum_{p<i} L(i,p) x_p).   SB = block edge (32, 64 or 128).
 template <int SB>
-__global__ void __launch_bounds__(256) forward_solve_kernel(const double* __restrict__ L, int t, int NB,
-                                                            const double* __restrict__ invD, const double* __restrict__ y,
-                                                            double* __restrict__ x, int* __restrict__ flags,
-                                                            unsigned int* __restrict__ ticket) {
-    constexpr int TX = SB / 4;            // threads across a row (4 columns each)
-    constexpr int TY = 256 / TX;          // row groups
-    constexpr int RPT = SB / TY;          // rows per thread
-    __shared__ double s_red[SB * (TX + 1)];
-    __shared__ double s_rhs[SB];
+struct SolveCfg {
+    static constexpr int TX = SB / 4;             // threads across a row (4 columns each); divides 32
+    static constexpr int TY = 256 / TX;           // row groups
+    static constexpr int RPT = SB / TY;           // rows per thread
+    static constexpr int kSmemBytes = SB * SB * 8 + SB * 8 + TY * SB * 8;   // invD, rhs, cross-warp partials
+};
+
+// sum over the TX lanes that share a row group (TX is a power of two <= 32, groups are lane-aligned)
+template <int TX>
+__device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+    for (int o = TX / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Forward: x_i = invD_i (y_i - sum_{p<i} L(i,p) x_p).
+template <int SB>
+__global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __restrict__ L, int t, int NB,
+                                                               const double* __restrict__ invD, const double* __restrict__ y,
+                                                               double* x, int* flags, unsigned int* ticket) {
+    using Cfg = SolveCfg<SB>;
+    constexpr int TX = Cfg::TX, TY = Cfg::TY, RPT = Cfg::RPT;
+    extern __shared__ __align__(16) double sm[];
+    double* s_inv = sm;                 // SB x SB, row-major
+    double* s_rhs = sm + SB * SB;       // SB
     __shared__ unsigned int s_row;
-    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX, lane = tid & 31;
     const int sbt = t / SB;
     if (tid == 0) s_row = atomicAdd(ticket, 1u);
     __syncthreads();
     const int i = (int)s_row;
     if (i >= NB) return;
+    {   // (a) the inverted diagonal block, in the background
+        const double* inv = invD + (size_t)i * SB * SB;
+        for (int idx = tid; idx < SB * SB / 2; idx += 256) cp_async16_solve(s_inv + 2 * idx, inv + 2 * idx);
+    }
     double acc[RPT];
 #pragma unroll
     for (int r = 0; r < RPT; ++r) acc[r] = 0.0;
     for (int pb = 0; pb < i; ++pb) {
-        if (tid == 0) { while (ld_acquire_i(flags + pb) == 0) __nanosleep(32); }
-        __syncthreads();
         const double* blk = tile_block_ptr(L, t, sbt, i, pb, SB);
+        double2 l[RPT][2];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {      // (b) the block of L first ...
+            const double2* row = reinterpret_cast<const double2*>(blk + (size_t)(ty + TY * r) * t + 4 * tx);
+            l[r][0] = __ldcs(row);
+            l[r][1] = __ldcs(row + 1);
+        }
+        if (lane == 0) {                     // (c) ... then the wait for x_p, per warp
+            while (ld_acquire_i(flags + pb) == 0) __nanosleep(20);
+        }
+        __syncwarp();
         const double2 x01 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx));
         const double2 x23 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx + 2));
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
-            const double* row = blk + (size_t)(ty + TY * r) * t + 4 * tx;
-            const double2 l01 = __ldcs(reinterpret_cast<const double2*>(row));
-            const double2 l23 = __ldcs(reinterpret_cast<const double2*>(row) + 1);
-            acc[r] = fma(l01.x, x01.x, acc[r]);
-            acc[r] = fma(l01.y, x01.y, acc[r]);
-            acc[r] = fma(l23.x, x23.x, acc[r]);
-            acc[r] = fma(l23.y, x23.y, acc[r]);
+            acc[r] = fma(l[r][0].x, x01.x, acc[r]);
+            acc[r] = fma(l[r][0].y, x01.y, acc[r]);
+            acc[r] = fma(l[r][1].x, x23.x, acc[r]);
+            acc[r] = fma(l[r][1].y, x23.y, acc[r]);
         }
     }
-    // reduce the TX partial sums of every row
 #pragma unroll
-    for (int r = 0; r < RPT; ++r) s_red[(ty + TY * r) * (TX + 1) + tx] = acc[r];
-    __syncthreads();
-    if (tid < SB) {
-        double s = 0.0;
-        for (int k = 0; k < TX; ++k) s += s_red[tid * (TX + 1) + k];
-        s_rhs[tid] = y[(size_t)i * SB + tid] - s;
+    for (int r = 0; r < RPT; ++r) acc[r] = group_sum<TX>(acc[r]);
+    if (tx == 0) {
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) s_rhs[ty + TY * r] = y[(size_t)i * SB + ty + TY * r] - acc[r];
     }
+    cp_async_wait_all_solve();
     __syncthreads();
-    // x_i = invD_i * rhs  (lower triangular inverse, row-major SB x SB)
-    const double* inv = invD + (size_t)i * SB * SB;
+    // x_i = invD_i * rhs  (lower triangular inverse; its strict upper part is stored as zeros)
     double part[RPT];
 #pragma unroll
     for (int r = 0; r < RPT; ++r) {
-        const double* row = inv + (size_t)(ty + TY * r) * SB + 4 * tx;
-        const double2 l01 = *reinterpret_cast<const double2*>(row);
-        const double2 l23 = *(reinterpret_cast<const double2*>(row) + 1);
-        part[r] = l01.x * s_rhs[4 * tx] + l01.y * s_rhs[4 * tx + 1] + l23.x * s_rhs[4 * tx + 2] + l23.y * s_rhs[4 * tx + 3];
+        const double* row = s_inv + (size_t)(ty + TY * r) * SB + 4 * tx;
+        part[r] = row[0] * s_rhs[4 * tx] + row[1] * s_rhs[4 * tx + 1] + row[2] * s_rhs[4 * tx + 2] + row[3] * s_rhs[4 * tx + 3];
     }
-    __syncthreads();
 #pragma unroll
-    for (int r = 0; r < RPT; ++r) s_red[(ty + TY * r) * (TX + 1) + tx] = part[r];
-    __syncthreads();
-    if (tid < SB) {
-        double s = 0.0;
-        for (int k = 0; k < TX; ++k) s += s_red[tid * (TX + 1) + k];
-        x[(size_t)i * SB + tid] = s;
+    for (int r = 0; r < RPT; ++r) part[r] = group_sum<TX>(part[r]);
+    if (tx == 0) {
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) x[(size_t)i * SB + ty + TY * r] = part[r];
     }
     __threadfence();
     __syncthreads();
@@ -223,71 +251,79 @@ __global__ void __launch_bounds__(256) forward_solve_kernel(const double* __rest
 
 // Backward: x_j = invD_j^T (b_j - sum_{i>j} L(i,j)^T x_i); block columns handed out from the last.
 template <int SB>
-__global__ void __launch_bounds__(256) backward_solve_kernel(const double* __restrict__ L, int t, int NB,
-                                                             const double* __restrict__ invD, const double* __restrict__ b,
-                                                             double* __restrict__ x, int* __restrict__ flags,
-                                                             unsigned int* __restrict__ ticket) {
-    constexpr int TX = SB / 4;
-    constexpr int TY = 256 / TX;
-    constexpr int RPT = SB / TY;
-    __shared__ double s_red[TY * SB];
-    __shared__ double s_rhs[SB];
+__global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __restrict__ L, int t, int NB,
+                                                                const double* __restrict__ invD, const double* __restrict__ b,
+                                                                double* x, int* flags, unsigned int* ticket) {
+    using Cfg = SolveCfg<SB>;
+    constexpr int TX = Cfg::TX, TY = Cfg::TY, RPT = Cfg::RPT;
+    extern __shared__ __align__(16) double sm[];
+    double* s_inv = sm;                          // SB x SB, row-major
+    double* s_rhs = sm + SB * SB;                // SB
+    double* s_part = sm + SB * SB + SB;          // TY x SB partial column sums
     __shared__ unsigned int s_col;
-    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX, lane = tid & 31;
     const int sbt = t / SB;
     if (tid == 0) s_col = atomicAdd(ticket, 1u);
     __syncthreads();
     if ((int)s_col >= NB) return;
     const int j = NB - 1 - (int)s_col;
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};     // columns 4tx..4tx+3, partial over this thread's rows
+    {
+        const double* inv = invD + (size_t)j * SB * SB;
+        for (int idx = tid; idx < SB * SB / 2; idx += 256) cp_async16_solve(s_inv + 2 * idx, inv + 2 * idx);
+    }
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};        // columns 4tx..4tx+3, partial over this thread's rows
     for (int ib = NB - 1; ib > j; --ib) {
-        if (tid == 0) { while (ld_acquire_i(flags + ib) == 0) __nanosleep(32); }
-        __syncthreads();
         const double* blk = tile_block_ptr(L, t, sbt, ib, j, SB);
+        double2 l[RPT][2];
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
-            const int rr = ty + TY * r;
-            const double xv = __ldcg(x + (size_t)ib * SB + rr);
-            const double* row = blk + (size_t)rr * t + 4 * tx;
-            const double2 l01 = __ldcs(reinterpret_cast<const double2*>(row));
-            const double2 l23 = __ldcs(reinterpret_cast<const double2*>(row) + 1);
-            acc[0] = fma(l01.x, xv, acc[0]);
-            acc[1] = fma(l01.y, xv, acc[1]);
-            acc[2] = fma(l23.x, xv, acc[2]);
-            acc[3] = fma(l23.y, xv, acc[3]);
+            const double2* row = reinterpret_cast<const double2*>(blk + (size_t)(ty + TY * r) * t + 4 * tx);
+            l[r][0] = __ldcs(row);
+            l[r][1] = __ldcs(row + 1);
+        }
+        if (lane == 0) {
+            while (ld_acquire_i(flags + ib) == 0) __nanosleep(20);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const double xv = __ldcg(x + (size_t)ib * SB + ty + TY * r);
+            acc[0] = fma(l[r][0].x, xv, acc[0]);
+            acc[1] = fma(l[r][0].y, xv, acc[1]);
+            acc[2] = fma(l[r][1].x, xv, acc[2]);
+            acc[3] = fma(l[r][1].y, xv, acc[3]);
         }
     }
 #pragma unroll
-    for (int c = 0; c < 4; ++c) s_red[ty * SB + 4 * tx + c] = acc[c];
+    for (int c = 0; c < 4; ++c) s_part[ty * SB + 4 * tx + c] = acc[c];
+    cp_async_wait_all_solve();
     __syncthreads();
     if (tid < SB) {
         double s = 0.0;
-        for (int k = 0; k < TY; ++k) s += s_red[k * SB + tid];
+#pragma unroll
+        for (int k = 0; k < TY; ++k) s += s_part[k * SB + tid];
         s_rhs[tid] = b[(size_t)j * SB + tid] - s;
     }
     __syncthreads();
     // x_j = invD_j^T rhs:  x[c] = sum_r inv[r][c] rhs[r]
-    const double* inv = invD + (size_t)j * SB * SB;
     double part[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int r = 0; r < RPT; ++r) {
         const int rr = ty + TY * r;
         const double rv = s_rhs[rr];
-        const double* row = inv + (size_t)rr * SB + 4 * tx;
-        const double2 l01 = *reinterpret_cast<const double2*>(row);
-        const double2 l23 = *(reinterpret_cast<const double2*>(row) + 1);
-        part[0] = fma(l01.x, rv, part[0]);
-        part[1] = fma(l01.y, rv, part[1]);
-        part[2] = fma(l23.x, rv, part[2]);
-        part[3] = fma(l23.y, rv, part[3]);
+        const double* row = s_inv + (size_t)rr * SB + 4 * tx;
+        part[0] = fma(row[0], rv, part[0]);
+        part[1] = fma(row[1], rv, part[1]);
+        part[2] = fma(row[2], rv, part[2]);
+        part[3] = fma(row[3], rv, part[3]);
     }
-    __syncthreads();
 #pragma unroll
-    for (int c = 0; c < 4; ++c) s_red[ty * SB + 4 * tx + c] = part[c];
+    for (int c = 0; c < 4; ++c) s_part[ty * SB + 4 * tx + c] = part[c];
     __syncthreads();
     if (tid < SB) {
         double s = 0.0;
-        for (int k = 0; k < TY; ++k) s += s_red[k * SB + tid];
+#pragma unroll
+        for (int k = 0; k < TY; ++k) s += s_part[k * SB + tid];
         x[(size_t)j * SB + tid] = s;
     }
     __threadfence();

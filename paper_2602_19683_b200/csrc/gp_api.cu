@@ -41,7 +41,8 @@ bool hyper_ok(const gp_hyper& h) {
 
 HyperDev to_dev(const gp_hyper& h) {
     HyperDev d;
-    d.den = h.ell_squared ? 2.0 * h.lengthscale * h.lengthscale : 2.0 * h.lengthscale;
+    const double den = h.ell_squared ? 2.0 * h.lengthscale * h.lengthscale : 2.0 * h.lengthscale;
+    d.neg_inv_den = -1.0 / den;
     d.vertical = h.vertical;
     d.noise = h.noise;
     return d;

@@ -8,13 +8,46 @@
 namespace gpb {
 
 struct HyperDev {
-    double den;       // 2*ell (Eq. 1 as printed) or 2*ell^2 (reading A1)
+    double neg_inv_den;   // -1/den, den = 2*ell (Eq. 1 as printed) or 2*ell^2 (reading A1); formed once on the host:
+                          // an FP64 division per matrix entry (~25 instructions, more than the exp) made the
+                          // assembly issue-bound; exact for den a power of two (ell = 1, 2), else <= 1 ulp in the exponent
     double vertical;  // v
     double noise;     // sigma^2
 };
 
+// exp(x) for x <= 0, the only range Eq. 1 needs (x = -r^2/den).  The library exp() carries
+// special-case branches and selects that made the assembly ISSUE-bound (ncu: issue slots 77 % busy,
+// FP64 pipe 54 %); this is the same algorithm without them: k = round(x log2 e) by the 1.5*2^52 trick,
+// f = x - k ln2 in two FMAs (|f| <= 0.347), degree-13 Taylor polynomial in Horner form (truncation
+// 4e-18 relative), 2^k added into the exponent field.  Error ~1 ulp, like the library's.  Results
+// below 2^-1021 (x < -708) are flushed to 0: an absolute error of 3e-308.
+__device__ __forceinline__ double exp_nonpos(double x) {
+    const double kMagic = 6755399441055744.0;                  // 1.5 * 2^52
+    const double t = fma(x, 1.4426950408889634, kMagic);
+    const int k = __double2loint(t);                           // round(x * log2 e), two's complement in the low word
+    const double kd = t - kMagic;
+    double f = fma(kd, -6.93147180369123816490e-01, x);        // ln2 high part (21 trailing zero bits)
+    f = fma(kd, -1.90821492927058770002e-10, f);               // ln2 low part
+    double p = 1.6059043836821613e-10;                         // 1/13!
+    p = fma(p, f, 2.08767569878681e-09);                       // 1/12!
+    p = fma(p, f, 2.505210838544172e-08);                      // 1/11!
+    p = fma(p, f, 2.755731922398589e-07);                      // 1/10!
+    p = fma(p, f, 2.7557319223985893e-06);                     // 1/9!
+    p = fma(p, f, 2.48015873015873e-05);                       // 1/8!
+    p = fma(p, f, 1.984126984126984e-04);                      // 1/7!
+    p = fma(p, f, 1.388888888888889e-03);                      // 1/6!
+    p = fma(p, f, 8.333333333333333e-03);                      // 1/5!
+    p = fma(p, f, 4.1666666666666664e-02);                     // 1/4!
+    p = fma(p, f, 1.6666666666666666e-01);                     // 1/3!
+    p = fma(p, f, 0.5);
+    p = fma(p, f, 1.0);
+    p = fma(p, f, 1.0);
+    const double r = __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+    return (x < -708.0) ? 0.0 : r;
+}
+
 // k(a,b) without the noise term -- PAPER.md:63, Eq. 1.  r2 accumulated in index order with FMA.
-__device__ __forceinline__ double se_kernel(double r2, const HyperDev& h) { return h.vertical * exp(-r2 / h.den); }
+__device__ __forceinline__ double se_kernel(double r2, const HyperDev& h) { return h.vertical * exp_nonpos(r2 * h.neg_inv_den); }
 
 // ---------------------------------------------------------------------------------------------
 // Fused assembly: distance, exp, noise in one pass, one 64x64 output sub-block per CTA.
@@ -83,15 +116,18 @@ __global__ void __launch_bounds__(256) assemble_tiles_kernel(const double* __res
         }
     }
     double* tbase = out + (size_t)tidx * tile * tile;
+    const bool on_diagonal = sym_lower && gi0 == gj0;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int r = ty + 16 * i;
         if (r >= nrow || 4 * tx >= ncol) continue;
         double k[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            k[j] = se_kernel(acc[i][j], h);
-            if (sym_lower && (gi0 + r) == (gj0 + 4 * tx + j)) k[j] += h.noise;
+        for (int j = 0; j < 4; ++j) k[j] = se_kernel(acc[i][j], h);
+        if (on_diagonal) {      // CTA-uniform: only sub-blocks that straddle the global diagonal carry noise
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (r == 4 * tx + j) k[j] += h.noise;
         }
         double* dst = tbase + (size_t)(r0 + r) * tile + c0 + 4 * tx;
         __stcs(reinterpret_cast<double2*>(dst), make_double2(k[0], k[1]));

@@ -313,6 +313,22 @@ def run_b200(args):
     total_ms = sum(events[s][0].elapsed_time(events[s][5]) for s in range(args.steps))
     per_step_chol = [events[s][1].elapsed_time(events[s][2]) for s in range(args.steps)]
 
+    # SURVEY.md 8(f) rows 1 and 4, outside the step (reported next to it): variance-only prediction given L and
+    # the log marginal likelihood, median of 3 after one warm-up
+    var = torch.empty(m, dtype=torch.float64, device="cuda")
+    lml = torch.empty(1, dtype=torch.float64, device="cuda")
+    tv, tl = [], []
+    for r in range(4):
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        e[0].record(); gp.gp_predict_variance(pipe.KL, dX, dXs, h, tile, args.width, var, pipe.work)
+        e[1].record(); gp.gp_log_marginal_likelihood(pipe.KL, n, tile, dY, pipe.alpha, lml)
+        e[2].record(); torch.cuda.synchronize()
+        if r > 0:
+            tv.append(e[0].elapsed_time(e[1])); tl.append(e[1].elapsed_time(e[2]))
+    next_rows = {"predict_variance_ms": statistics.median(tv), "log_marginal_likelihood_ms": statistics.median(tl),
+                 "log_marginal_likelihood": float(lml.item()), "variance_min_max": [float(var.min().item()), float(var.max().item())]}
+    del var, lml
+
     # end to end through the host-buffer C-ABI call: H2D of X, y, X^ and D2H of mean, Sigma inside
     ws = torch.empty(gp.gp_pipeline_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
     hMean = torch.empty(m, dtype=torch.float64).pin_memory()
@@ -369,6 +385,7 @@ def run_b200(args):
                          "assemble_gbs": (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["assemble"] * 1e-3) / 1e9,
                          "solve_gbs": 2 * (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["solve"] * 1e-3) / 1e9},
             "clocks": clocks,
+            "next_rows": next_rows,
         }
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(cfg)

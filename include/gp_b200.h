@@ -121,6 +121,22 @@ int gp_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* chol, size
 int gp_tiles_to_dense(const double* dTiles, int64_t n, int64_t nb, int tile, int lower_packed,
                       double* dDense, void* stream);
 
+/* SURVEY.md 8(f) row 1, "predict with uncertainty" ("the diagonal elements of Sigma
+ * represent the predictive variances"): dVar[m] <- diag(Sigma) = k(x^,x^) - sum_i V_i^2 without the
+ * n m^2 contraction W = V^T V and without the m x m output.  Same arguments, workspace (the m x n
+ * V^T buffer; size = full_cov of gp_workspace_bytes) and error behaviour as gp_predict_full_cov;
+ * the prior variance is noise-free (reading A2), so 0 <= dVar[a] <= v. */
+int gp_predict_variance(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m,
+                        gp_hyper h, int tile, int sched_width, double* dVar, void* dWork, size_t work_bytes,
+                        void* stream);
+
+/* SURVEY.md 8(f) row 4 (hyperparameters "are typically subject to optimization"): the
+ * objective of that optimisation, *d_out (device double) <- log p(y) = -1/2 y^T alpha - sum_i log L_ii
+ * - n/2 log(2 pi), from the factor of gp_cholesky_tiled and the alpha of gp_solve.  One CTA, fixed
+ * summation order (bitwise reproducible). */
+int gp_log_marginal_likelihood(const double* dL, int64_t n, int tile, const double* dY, const double* dAlpha,
+                               double* d_out, void* stream);
+
 /* Number of tile tasks (POTRF + TRSM + SYRK + GEMM) and of CTA-sized work items the scheduler
  * runs for an n x n factorisation with this tile size (a6 bookkeeping; host only). */
 int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* work_items);
@@ -178,6 +194,8 @@ int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* s
  * its final version, GP_ERR_SIZE otherwise.  stats (may be NULL) receives
  * {items, dependency edges, simulated makespan us, total work us, critical path us}. */
 int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5);
+/* The same for the schedule of gp_predict_variance (m > 0; no W = V^T V items). */
+int gp_schedule_selfcheck_variance(int64_t n, int64_t m, int tile, int workers, double* stats5);
 
 /* Drop the cached device-resident schedules (synchronises the device). */
 void gp_release_cached_schedules(void);

@@ -58,6 +58,9 @@ def _load():
         lib.oracle_forward_subst_cols.argtypes = [dp, i64, dp, i64, dp]
         lib.oracle_posterior_cov.argtypes = [dp, i64, i64, dp, dp]
         lib.oracle_dense_matvec.argtypes = [dp, i64, dp, dp]
+        lib.oracle_posterior_var.argtypes = [dp, i64, i64, dp, dp]
+        lib.oracle_log_marginal_likelihood.argtypes = [dp, i64, dp, dp]
+        lib.oracle_log_marginal_likelihood.restype = ctypes.c_double
         _lib = lib
     return _lib
 
@@ -166,6 +169,23 @@ def posterior_cov(V: np.ndarray, Kss: np.ndarray) -> np.ndarray:
     return S
 
 
+def posterior_var(V: np.ndarray, kss_diag: np.ndarray) -> np.ndarray:
+    """diag(Sigma): var_a = k(x^_a, x^_a) - sum_i V_ia^2."""
+    V = _c(V)
+    n, m = V.shape
+    kss_diag = _c(kss_diag, (m,))
+    var = np.empty(m, dtype=np.float64)
+    _load().oracle_posterior_var(_p(V), n, m, _p(kss_diag), _p(var))
+    return var
+
+
+def log_marginal_likelihood(L: np.ndarray, y: np.ndarray, alpha: np.ndarray) -> float:
+    """log p(y) = -1/2 y^T alpha - sum_i log L_ii - n/2 log(2 pi)."""
+    L = _c(L)
+    n = L.shape[0]
+    return float(_load().oracle_log_marginal_likelihood(_p(L), n, _p(_c(y, (n,))), _p(_c(alpha, (n,)))))
+
+
 @dataclass
 class Prediction:
     K: np.ndarray | None
@@ -175,6 +195,7 @@ class Prediction:
     mean: np.ndarray | None = None
     V: np.ndarray | None = None
     Sigma: np.ndarray | None = None
+    var: np.ndarray | None = None
 
 
 def fit(X: np.ndarray, y: np.ndarray, h: Hyper, keep_K: bool = True) -> Prediction:
@@ -187,7 +208,7 @@ def fit(X: np.ndarray, y: np.ndarray, h: Hyper, keep_K: bool = True) -> Predicti
 
 
 def predict(X: np.ndarray, y: np.ndarray, Xs: np.ndarray, h: Hyper, full_cov: bool = True,
-            fitted: Prediction | None = None) -> Prediction:
+            fitted: Prediction | None = None, variance: bool = False) -> Prediction:
     """The whole pipeline of PAPER.md section 4.1 in the paper's order:
     K, L, beta, alpha, K_{X^,X}, mean, V, W, Sigma."""
     p = fitted if fitted is not None else fit(X, y, h)
@@ -197,4 +218,8 @@ def predict(X: np.ndarray, y: np.ndarray, Xs: np.ndarray, h: Hyper, full_cov: bo
         p.V = forward_subst_cols(p.L, np.ascontiguousarray(Kxs.T))   # L V = K_{X,X^}
         Kss = assemble(Xs, Xs, h, add_noise_diag=False)     # prior test covariance, noise-free
         p.Sigma = posterior_cov(p.V, Kss)                   # Eq. 3
+    if variance:                                            # "predict with uncertainty": the diagonal only
+        if p.V is None:
+            p.V = forward_subst_cols(p.L, np.ascontiguousarray(Kxs.T))
+        p.var = posterior_var(p.V, np.full(Xs.shape[0], h.vertical))   # k(x,x) = v exp(0), noise-free (A2)
     return p

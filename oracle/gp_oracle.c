@@ -196,3 +196,33 @@ void oracle_dense_matvec(const double *K, int64_t n, const double *x, double *y)
 {
     oracle_matvec(K, n, n, x, y);
 }
+
+/*
+ * "The diagonal elements of Sigma represent the predictive
+ * variances".  The diagonal of Eq. 3 written out, without forming W:
+ *   var[a] = kss_diag[a] - sum_{i=0}^{n-1} V[i][a]^2,   kss_diag[a] = k(x^_a, x^_a) (noise-free, A2),
+ * each sum in index order.  V is n x m.
+ */
+void oracle_posterior_var(const double *V, int64_t n, int64_t m, const double *kss_diag, double *var)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t a = 0; a < m; ++a) {
+        double w = 0.0;
+        for (int64_t i = 0; i < n; ++i) w += V[i * m + a] * V[i * m + a];
+        var[a] = kss_diag[a] - w;
+    }
+}
+
+/*
+ * SURVEY.md 8(f) row 4 ("hyperparameters are typically subject to optimization"): the
+ * objective of that optimisation, the log marginal likelihood of y ~ N(0, K), K = L L^T, alpha = K^-1 y:
+ *   log p(y) = -1/2 y^T alpha - sum_i log L_ii - n/2 log(2 pi)
+ * (log det K = 2 sum_i log L_ii).  Sums in index order, serial.
+ */
+double oracle_log_marginal_likelihood(const double *L, int64_t n, const double *y, const double *alpha)
+{
+    double quad = 0.0, logdiag = 0.0;
+    for (int64_t i = 0; i < n; ++i) quad += y[i] * alpha[i];
+    for (int64_t i = 0; i < n; ++i) logdiag += log(L[i * n + i]);
+    return -0.5 * quad - logdiag - 0.5 * (double)n * log(2.0 * 3.14159265358979323846264338327950288);
+}

@@ -22,7 +22,8 @@ ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA":
 EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
-           "gp_contraction_bench_launch")
+           "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
+           "gp_schedule_selfcheck_variance")
 
 
 class gp_hyper(ctypes.Structure):
@@ -66,6 +67,8 @@ def load() -> ctypes.CDLL:
     lib.gp_solve.argtypes = [vp, i64, ci, vp, vp, vp, vp, sz, vp]
     lib.gp_predict_mean.argtypes = [vp, i64, ci, vp, vp, i64, gp_hyper, vp, vp]
     lib.gp_predict_full_cov.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
+    lib.gp_predict_variance.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
+    lib.gp_log_marginal_likelihood.argtypes = [vp, i64, ci, vp, vp, vp, vp]
     lib.gp_workspace_bytes.argtypes = [i64, i64, ci, ci, psz, psz, psz]
     lib.gp_tiles_to_dense.argtypes = [vp, i64, i64, ci, ci, vp, vp]
     lib.gp_cholesky_task_counts.argtypes = [i64, ci, ctypes.POINTER(i64), ctypes.POINTER(i64)]
@@ -76,6 +79,7 @@ def load() -> ctypes.CDLL:
     lib.gp_pipeline_workspace_bytes.argtypes = [i64, i64, ci, ci, psz]
     lib.gp_pipeline_host.argtypes = [vp, vp, vp, i64, i64, ci, gp_hyper, ci, ci, vp, vp, vp, vp, vp, sz, vp]
     lib.gp_schedule_selfcheck.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.gp_schedule_selfcheck_variance.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_exec_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ci, vp]
     lib.gp_fp64_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
@@ -163,6 +167,19 @@ def gp_predict_full_cov(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: H
                                       _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_full_cov")
 
 
+def gp_predict_variance(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
+                        var: torch.Tensor, work: torch.Tensor) -> None:
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_variance(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(var),
+                                      _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_variance")
+
+
+def gp_log_marginal_likelihood(L: torch.Tensor, n: int, tile: int, y: torch.Tensor, alpha: torch.Tensor, out: torch.Tensor) -> None:
+    _check(load().gp_log_marginal_likelihood(_ptr(L), n, tile, _ptr(y), _ptr(alpha), _ptr(out), _stream()),
+           "gp_log_marginal_likelihood")
+
+
 def gp_tiles_to_dense(tiles: torch.Tensor, n: int, nb: int, tile: int, lower_packed: bool, dense: torch.Tensor) -> torch.Tensor:
     _check(load().gp_tiles_to_dense(_ptr(tiles), n, nb, tile, int(lower_packed), _ptr(dense), _stream()), "gp_tiles_to_dense")
     return dense
@@ -211,7 +228,8 @@ def gp_contraction_bench_launch(K: int, reps: int, buf: torch.Tensor) -> float:
     """Enqueue one launch of the contraction steady-state microbenchmark; returns its flop count."""
     f = ctypes.c_double(0.0)
     _check(load().gp_contraction_bench_launch(K, reps, _ptr(buf, torch.uint8), buf.numel(), ctypes.byref(f), None, _stream()),
-           "gp_contraction_bench_launch")
+           "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
+           "gp_schedule_selfcheck_variance")
     return float(f.value)
 
 
@@ -219,6 +237,12 @@ def gp_schedule_selfcheck(n: int, m: int, tile: int, workers: int = 148):
     """(rc, stats) of the host-only schedule replay; stats = items, edges, makespan_us, work_us, critical_path_us."""
     st = (ctypes.c_double * 5)()
     rc = int(load().gp_schedule_selfcheck(n, m, tile, workers, st))
+    return rc, dict(zip(("items", "edges", "makespan_us", "work_us", "critical_path_us"), list(st)))
+
+
+def gp_schedule_selfcheck_variance(n: int, m: int, tile: int, workers: int = 148):
+    st = (ctypes.c_double * 5)()
+    rc = int(load().gp_schedule_selfcheck_variance(n, m, tile, workers, st))
     return rc, dict(zip(("items", "edges", "makespan_us", "work_us", "critical_path_us"), list(st)))
 
 

@@ -81,7 +81,7 @@ int get_schedule(int kind, int M, int Mm, int nbt, int blk, int workers, CachedS
     if (it != g_cache.end()) { *out = it->second; return GP_OK; }
     std::vector<SchedItem> items;
     if (kind == 0) build_cholesky_schedule(M, nbt, workers, items, blk);
-    else build_predict_schedule(M, Mm, nbt, workers, items, blk);
+    else build_predict_schedule(M, Mm, nbt, workers, items, blk, nullptr, true, /*with_sigma=*/kind == 1);
     static_assert(sizeof(SchedItem) == sizeof(Item), "schedule item layout");
     CachedSchedule cs;
     cs.nitems = (int)items.size();
@@ -402,9 +402,10 @@ int gp_predict_mean(const double* dX, int64_t n, int D, const double* dAlpha, co
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
-int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
-                        int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
-    if (!dL || !dX || !dXs || !dSigma || !dWork) return GP_ERR_NULL;
+// a9, a11, a12 (dSigma != NULL) or the variance-only variant (dSigma == NULL, dVar != NULL)
+static int run_predictor(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
+                         int sched_width, double* dSigma, double* dVar, void* dWork, size_t work_bytes, void* stream) {
+    if (!dL || !dX || !dXs || (!dSigma && !dVar) || !dWork) return GP_ERR_NULL;
     if (n <= 0 || m <= 0 || D <= 0 || n > (int64_t)1 << 22 || m > (int64_t)1 << 22) return GP_ERR_SIZE;
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
@@ -418,7 +419,7 @@ int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, co
     const int M = (int)(n / tile), Mm = (int)(m / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
     const int workers = workers_for(sched_width);
     CachedSchedule cs;
-    rc = get_schedule(1, M, Mm, nbt, b, sm_count(), &cs);
+    rc = get_schedule(dSigma ? 1 : 2, M, Mm, nbt, b, sm_count(), &cs);
     if (rc != GP_OK) return rc;
     char* ws = (char*)dWork;
     const HyperDev hd = to_dev(h);
@@ -428,7 +429,7 @@ int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, co
     // a9: K_{X^,X} (m x n, noise-free) straight into the V^T buffer; prior K_{X^,X^} straight into Sigma
     rc = launch_assemble(dXs, m, dX, n, D, hd, tile, 0, Vt, st);
     if (rc != GP_OK) return rc;
-    {
+    if (dSigma) {
         // dense m x m = one "tile" of edge m
         const int sb = (int)((m + kAsmBlk - 1) / kAsmBlk);
         if ((int64_t)sb * sb > 2147483647LL) return GP_ERR_SIZE;
@@ -460,8 +461,35 @@ int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, co
     p.L_final = 1;
     rc = launch_exec_any(b, p, m, workers, st);
     if (rc != GP_OK) return rc;
-    dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
-    mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
+    if (dSigma) {
+        dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
+        mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
+    } else {
+        // var_a = k(x^_a, x^_a) - sum_i V_ia^2 with k(x,x) = v (noise-free prior, reading A2): one warp per test point
+        posterior_var_kernel<<<(unsigned)((m + 7) / 8), 256, 0, st>>>(Vt, m, n, tile, hd.vertical, dVar);
+    }
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_predict_full_cov(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
+                        int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
+    if (!dSigma) return GP_ERR_NULL;
+    return run_predictor(dL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, nullptr, dWork, work_bytes, stream);
+}
+
+int gp_predict_variance(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
+                        int sched_width, double* dVar, void* dWork, size_t work_bytes, void* stream) {
+    if (!dVar) return GP_ERR_NULL;
+    return run_predictor(dL, dX, n, D, dXs, m, h, tile, sched_width, nullptr, dVar, dWork, work_bytes, stream);
+}
+
+int gp_log_marginal_likelihood(const double* dL, int64_t n, int tile, const double* dY, const double* dAlpha, double* d_out,
+                               void* stream) {
+    if (!dL || !dY || !dAlpha || !d_out) return GP_ERR_NULL;
+    if (n <= 0) return GP_ERR_SIZE;
+    const int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    log_marginal_likelihood_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(dL, n, tile, dY, dAlpha, d_out);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
@@ -620,7 +648,7 @@ extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_worke
     return cudaStreamSynchronize(st) == cudaSuccess ? w : GP_ERR_CUDA;
 }
 
-extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5) {
+static int schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, bool with_sigma, double* stats5) {
     if (n <= 0 || m < 0) return GP_ERR_SIZE;
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
@@ -630,7 +658,7 @@ extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers
     std::vector<SchedItem> items;
     SchedStats st;
     if (m == 0) build_cholesky_schedule(M, nbt, workers, items, b, &st, true);
-    else build_predict_schedule(M, Mm, nbt, workers, items, b, &st, true);
+    else build_predict_schedule(M, Mm, nbt, workers, items, b, &st, true, with_sigma);
     if (stats5) {
         stats5[0] = (double)items.size();
         stats5[1] = (double)st.edges;
@@ -639,6 +667,14 @@ extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers
         stats5[4] = st.critical_path_us;
     }
     const char* why = nullptr;
-    return validate_schedule(items, M, Mm, nbt, m > 0, &why) ? GP_OK : GP_ERR_SIZE;
+    return validate_schedule(items, M, Mm, nbt, m > 0, &why, with_sigma) ? GP_OK : GP_ERR_SIZE;
 }
 
+extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5) {
+    return schedule_selfcheck(n, m, tile, workers, true, stats5);
+}
+
+extern "C" int gp_schedule_selfcheck_variance(int64_t n, int64_t m, int tile, int workers, double* stats5) {
+    if (m <= 0) return GP_ERR_SIZE;
+    return schedule_selfcheck(n, m, tile, workers, false, stats5);
+}

@@ -167,6 +167,51 @@ __global__ void mirror_lower_kernel(double* __restrict__ S, int64_t m) {
     }
 }
 
+// Predictive variances: var_a = prior - sum_i V^T[a][i]^2 over the
+// general tiles of V^T (m x n).  One warp per test point, lanes stride the row, fixed reduction order.
+__global__ void __launch_bounds__(256) posterior_var_kernel(const double* __restrict__ Vt, int64_t m, int64_t n, int tile,
+                                                            double prior, double* __restrict__ var) {
+    const int lane = threadIdx.x & 31;
+    const int64_t a = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (a >= m) return;
+    const int64_t Mt = n / tile;
+    const double* rowbase = Vt + (a / tile) * Mt * (size_t)tile * tile + (a % tile) * (size_t)tile;
+    double s = 0.0;
+    for (int64_t J = 0; J < Mt; ++J) {
+        const double2* row = reinterpret_cast<const double2*>(rowbase + J * (size_t)tile * tile);
+        for (int c = lane; c < tile / 2; c += 32) {
+            const double2 v = __ldcs(row + c);
+            s = fma(v.x, v.x, s);
+            s = fma(v.y, v.y, s);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) var[a] = prior - s;
+}
+
+// log p(y) = -1/2 y^T alpha - sum_i log L_ii - n/2 log(2 pi).  One CTA, fixed order.
+__global__ void __launch_bounds__(1024) log_marginal_likelihood_kernel(const double* __restrict__ L, int64_t n, int tile,
+                                                                        const double* __restrict__ y, const double* __restrict__ alpha,
+                                                                        double* __restrict__ out) {
+    __shared__ double s_q[32], s_l[32];
+    double q = 0.0, ld = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 1024) {
+        q = fma(y[i], alpha[i], q);
+        const int64_t I = i / tile, r = i % tile;
+        ld += log(L[((size_t)I * (I + 1) / 2 + I) * (size_t)tile * tile + r * (size_t)tile + r]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { q += __shfl_xor_sync(0xffffffffu, q, o); ld += __shfl_xor_sync(0xffffffffu, ld, o); }
+    if ((threadIdx.x & 31) == 0) { s_q[threadIdx.x >> 5] = q; s_l[threadIdx.x >> 5] = ld; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tq = 0.0, tl = 0.0;
+        for (int k = 0; k < 32; ++k) { tq += s_q[k]; tl += s_l[k]; }
+        out[0] = -0.5 * tq - tl - 0.5 * (double)n * 1.8378770664093454835606594728112;   // log(2 pi)
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Triangular solves for alpha.  Block rows/columns of SB (= the executor's block
 // edge).  One CTA per block row; rows are handed out by a ticket so that a CTA only ever waits for

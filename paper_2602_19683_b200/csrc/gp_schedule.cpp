@@ -142,7 +142,7 @@ void program_order_cholesky(int M, int nbt, std::vector<SchedItem>& v, std::vect
     }
 }
 
-void program_order_predict(int M, int Mm, int nbt, std::vector<SchedItem>& v, std::vector<int32_t>& task) {
+void program_order_predict(int M, int Mm, int nbt, bool with_sigma, std::vector<SchedItem>& v, std::vector<int32_t>& task) {
     int32_t tid = 0;
     auto emit = [&](const SchedItem& it) { v.push_back(it); task.push_back(tid); };
     for (int J = 0; J < M; ++J) {
@@ -157,6 +157,7 @@ void program_order_predict(int M, int Mm, int nbt, std::vector<SchedItem>& v, st
                     for (int ba = 0; ba < nbt; ++ba) emit(mk(S_UPD_V, A * nbt + ba, P * nbt + bk, qt, qt + nbt));
                 ++tid;
             }
+        if (!with_sigma) continue;                                                                // variances only: no W
         for (int B = 0; B < Mm; ++B)                                                              // Sigma_{A,B} -= V^T_{A,J} V^T_{B,J}^T
             for (int A = B; A < Mm; ++A) {
                 for (int bb = 0; bb < nbt; ++bb)
@@ -286,14 +287,15 @@ void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>
     schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, stats, simulate);
 }
 
-void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate) {
+void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate,
+                            bool with_sigma) {
     std::vector<SchedItem> prog;
     std::vector<int32_t> task;
-    program_order_predict(M, Mm, nbt, prog, task);
+    program_order_predict(M, Mm, nbt, with_sigma, prog, task);
     schedule(Shape(M, Mm, nbt, true), prog, task, workers, blk, out, stats, simulate);
 }
 
-bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why) {
+bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why, bool with_sigma) {
     const Shape s(M, predict ? Mm : 0, nbt, predict);
     std::vector<int32_t> ver(s.nblocks, 0);
     static const char* kWait = "an item waits for a version no earlier item produces";
@@ -313,12 +315,12 @@ bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int n
             for (int gc = 0; gc < s.NB; ++gc)
                 if (ver[s.idV(gr, gc)] != s.finV(gc)) { if (why) *why = kFinal; return false; }
             for (int gc = 0; gc <= gr; ++gc)
-                if (ver[s.idS(gr, gc)] != M) { if (why) *why = kFinal; return false; }
+                if (ver[s.idS(gr, gc)] != (with_sigma ? M : 0)) { if (why) *why = kFinal; return false; }
         }
     }
     std::vector<SchedItem> prog;
     std::vector<int32_t> task;
-    if (predict) program_order_predict(M, Mm, nbt, prog, task); else program_order_cholesky(M, nbt, prog, task);
+    if (predict) program_order_predict(M, Mm, nbt, with_sigma, prog, task); else program_order_cholesky(M, nbt, prog, task);
     if (prog.size() != items.size()) { if (why) *why = kCount; return false; }
     return true;
 }

@@ -31,11 +31,13 @@ struct SchedStats {
 // M = n / tile, nbt = tile / block, Mm = m / tile.  `blk` (32/64/128) selects the cost model.
 void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>& out, int blk = 128,
                              SchedStats* stats = nullptr, bool simulate = true);
+// with_sigma = false leaves out the W = V^T V items (variance-only prediction).
 void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk = 128,
-                            SchedStats* stats = nullptr, bool simulate = true);
+                            SchedStats* stats = nullptr, bool simulate = true, bool with_sigma = true);
 
 // Checks that `items` is a valid execution order (every wait of every item is satisfied by items
 // earlier in the list) and that every block ends at its final version.  Used by the CPU tests.
-bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why);
+bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why,
+                       bool with_sigma = true);
 
 }  // namespace gpb

@@ -10,7 +10,7 @@ Run:  python tests/golden/make_worked_examples.py
 import json
 import os
 
-from mpmath import mp, mpf, exp, sqrt, matrix, inverse
+from mpmath import mp, mpf, exp, sqrt, matrix, inverse, det, log, pi
 
 mp.dps = 40
 
@@ -60,7 +60,12 @@ def example(X, y, Xs, ell, v, noise, ell_squared):
             V[i, c] = (Kxs[c, i] - sum(L[i, p] * V[p, c] for p in range(i))) / L[i, i]
     mean = Kxs * alpha
     Sigma = Kss - V.T * V
+    # log marginal likelihood of y ~ N(0, K) from the density itself (determinant and inverse), and its
+    # Cholesky form
+    lml_def = -(yv.T * Kinv * yv)[0] / 2 - log(det(K)) / 2 - mpf(n) / 2 * log(2 * pi)
+    lml = -(yv.T * alpha)[0] / 2 - sum(log(L[i, i]) for i in range(n)) - mpf(n) / 2 * log(2 * pi)
     tol = mpf(10) ** -35
+    assert abs(lml - lml_def) < tol
     assert max(abs(alpha[i] - alpha_inv[i]) for i in range(n)) < tol
     assert max(abs(mean[a] - mean_inv[a]) for a in range(m)) < tol
     assert max(abs(Sigma[a, b] - Sigma_inv[a, b]) for a in range(m) for b in range(m)) < tol
@@ -74,7 +79,8 @@ def example(X, y, Xs, ell, v, noise, ell_squared):
     return {"X": X, "y": y, "Xs": Xs, "lengthscale": ell, "vertical": v, "noise": noise,
             "ell_squared": bool(ell_squared), "K": mat(K), "L": mat(L), "beta": vec(beta),
             "alpha": vec(alpha), "K_X_Xs": mat(Kxs.T), "V": mat(V), "mean": vec(mean),
-            "Sigma": mat(Sigma)}
+            "Sigma": mat(Sigma), "var": [mp.nstr(Sigma_inv[a, a], 25) for a in range(m)],
+            "log_marginal_likelihood": mp.nstr(lml_def, 25)}
 
 
 def main():

@@ -3,6 +3,8 @@ full against the oracle; config 3 = the headline n=32768, m=4096, tile 1024 thro
 and sampled outputs, SURVEY.md section 8(c) "where the full oracle is too slow").  Only oracle
 code produces expected values; the GPU's L enters the Sigma check only after the residual test
 has pinned it (L is unique, reading A6)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -49,7 +51,18 @@ def test_config2_full_oracle(gp):
 
 
 def test_config3_headline_properties_and_samples(gp):
-    cfg = nfir.CONFIGS[3]
+    _properties_and_samples(gp, nfir.CONFIGS[3])
+
+
+@pytest.mark.skipif(os.environ.get("GP_B200_RUN_C4") != "1",
+                    reason="config 4 (n=65536) needs ~40 GB of host RAM and several minutes: set GP_B200_RUN_C4=1")
+def test_config4_largest_properties_and_samples(gp):
+    """The same property / sampled-output parity at the largest single-GPU configuration (tile 2048,
+    16 blocks per tile edge, D=16, lengthscale 2 with the as-printed exponent)."""
+    _properties_and_samples(gp, nfir.CONFIGS[4])
+
+
+def _properties_and_samples(gp, cfg):
     n, m = cfg.n, cfg.m
     X, y, Xs = nfir.make_inputs(cfg)
     h = oracle.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)

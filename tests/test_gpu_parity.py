@@ -206,3 +206,48 @@ def test_fp64_peak_probe_launches(gp):
         assert flops > 0
     torch.cuda.synchronize()
     assert float(sink.item()) == 0.0
+
+
+# ---------------------------------------------------------------- SURVEY.md 8(f) rows 1 and 4
+@pytest.mark.parametrize("n,m,D,tile", [(128, 128, 8, 32), (1024, 1024, 8, 256), (768, 256, 5, 128), (1280, 512, 16, 256)])
+def test_variance_only_and_log_marginal_likelihood(gp, n, m, D, tile):
+    """gp_predict_variance (diag Sigma without W) and gp_log_marginal_likelihood against the oracle."""
+    X, y = nfir.nfir_features(31, n, D)
+    Xs, _ = nfir.nfir_features(32, m, D, with_targets=False)
+    h = oracle.Hyper(2.0, 1.3, 0.05) if D == 16 else oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h, full_cov=True, variance=True)
+    hg = gp.Hyper(h.lengthscale, h.vertical, h.noise, h.ell_squared)
+    pipe = gp.GpPipeline(n, m, D, tile, hg)
+    dX, dy, dXs = _dev(X), _dev(y), _dev(Xs)
+    pipe.assemble(dX); pipe.cholesky(); pipe.solve(dy)
+    var = torch.empty(m, dtype=torch.float64, device="cuda")
+    gp.gp_predict_variance(pipe.KL, dX, dXs, hg, tile, 0, var, pipe.work)
+    lml = torch.empty(1, dtype=torch.float64, device="cuda")
+    gp.gp_log_marginal_likelihood(pipe.KL, n, tile, dy, pipe.alpha, lml)
+    # the full covariance afterwards, on the same workspace: its diagonal must agree with the variance path
+    gp.gp_predict_full_cov(pipe.KL, dX, dXs, hg, tile, 0, pipe.Sigma, pipe.work)
+    torch.cuda.synchronize()
+    assert int(pipe.info.item()) == 0
+    v = var.cpu().numpy()
+    assert relerr(v, p.var) <= TOL_SIGMA
+    np.testing.assert_allclose(v, p.var, rtol=0, atol=1e-9 * np.abs(p.var).max())
+    assert v.min() >= 0.0 and v.max() <= h.vertical
+    np.testing.assert_allclose(v, np.diag(pipe.Sigma.cpu().numpy()), rtol=0, atol=1e-12)
+    want = oracle.log_marginal_likelihood(p.L, y, p.alpha)
+    assert abs(float(lml.item()) - want) <= 1e-10 * abs(want)
+
+
+def test_variance_argument_errors(gp):
+    n, m, D, tile = 128, 128, 4, 32
+    X = torch.zeros(n, D, dtype=torch.float64, device="cuda")
+    pipe = gp.GpPipeline(n, m, D, tile, gp.Hyper())
+    var = torch.empty(m, dtype=torch.float64, device="cuda")
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_predict_variance(pipe.KL, X, X, gp.Hyper(), 48, 0, var, pipe.work)
+    assert e.value.code == gp.ERR["TILE"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_predict_variance(pipe.KL, X, X, gp.Hyper(), tile, 0, var, pipe.work[:1024])
+    assert e.value.code == gp.ERR["WORKSPACE"]
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_log_marginal_likelihood(pipe.KL, n, 48, pipe.alpha, pipe.alpha, var)
+    assert e.value.code == gp.ERR["TILE"]

@@ -82,6 +82,14 @@ def test_schedule_is_a_valid_topological_order(gp, n, m, tile, workers):
     assert st["makespan_us"] >= st["work_us"] / workers * 0.999
 
 
+@pytest.mark.parametrize("n,m,tile", [(128, 128, 32), (1024, 1024, 256), (1536, 384, 384), (8192, 1024, 1024), (4096, 1024, 128)])
+def test_variance_only_schedule_is_a_valid_topological_order(gp, n, m, tile):
+    rc, st = gp.gp_schedule_selfcheck_variance(n, m, tile, 148)
+    rc_full, st_full = gp.gp_schedule_selfcheck(n, m, tile, 148)
+    assert rc == 0 and rc_full == 0
+    assert 0 < st["items"] < st_full["items"]          # the W = V^T V items are gone
+
+
 def test_schedule_headline_config(gp):
     rc, st = gp.gp_schedule_selfcheck(32768, 0, 1024, 148)
     assert rc == 0

@@ -250,3 +250,59 @@ def test_oracle_thread_count_does_not_change_results():
         oracle.set_num_threads(nt)
     for a, b in ((p.L, q.L), (p.alpha, q.alpha), (p.mean, q.mean), (p.Sigma, q.Sigma)):
         assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------- SURVEY.md 8(f) rows 1 and 4
+@pytest.mark.parametrize("name", ["A", "B", "Bprime_printed_2ell", "Bprime_ell_squared"])
+def test_variance_and_lml_worked_examples_40_digits(golden, name):
+    """diag(Sigma) and log p(y) against the 40-digit values the golden script derives from
+    the DEFINITIONS (direct inverse, determinant), not from a Cholesky factor."""
+    g = golden[name]
+    h = Hyper(g["lengthscale"], g["vertical"], g["noise"], g["ell_squared"])
+    X, y, Xs = np.array(g["X"]), np.array(g["y"]), np.array(g["Xs"])
+    p = oracle.predict(X, y, Xs, h, full_cov=False, variance=True)
+    assert p.Sigma is None
+    np.testing.assert_allclose(p.var, _fv(g["var"]), rtol=1e-13, atol=1e-15)
+    lml = oracle.log_marginal_likelihood(p.L, y, p.alpha)
+    assert abs(lml - float(g["log_marginal_likelihood"])) <= 1e-13 * abs(float(g["log_marginal_likelihood"]))
+
+
+def test_lml_single_point_closed_form():
+    """n = 1: log N(y; 0, v + s2) = -y^2 / (2 (v + s2)) - log(v + s2) / 2 - log(2 pi) / 2."""
+    for v, s2, yv in ((1.0, 0.1, 0.7), (2.5, 0.05, -1.3)):
+        h = Hyper(1.0, v, s2)
+        p = oracle.fit(np.array([[0.3, -0.2]]), np.array([yv]), h)
+        want = -yv * yv / (2 * (v + s2)) - 0.5 * np.log(v + s2) - 0.5 * np.log(2 * np.pi)
+        assert abs(oracle.log_marginal_likelihood(p.L, np.array([yv]), p.alpha) - want) <= 1e-15 * max(1.0, abs(want))
+
+
+@pytest.mark.parametrize("n,m,D,seed", [(3, 2, 1, 0), (16, 9, 3, 1), (64, 40, 8, 2)])
+def test_variance_and_lml_brute_force_and_scipy(n, m, D, seed):
+    from scipy.stats import multivariate_normal
+    X, y = nfir.nfir_features(seed, n, D)
+    Xs, _ = nfir.nfir_features(seed + 50, m, D, with_targets=False)
+    for h in (Hyper(), Hyper(2.0, 1.0, 0.05), Hyper(2.0, 1.7, 0.05, True)):
+        p = oracle.predict(X, y, Xs, h, full_cov=True, variance=True)
+        K = se_kernel_numpy(X, X, h.lengthscale, h.vertical, h.ell_squared) + h.noise * np.eye(n)
+        Kxs = se_kernel_numpy(Xs, X, h.lengthscale, h.vertical, h.ell_squared)
+        Kinv = gauss_jordan_inverse(K)
+        # variance: the diagonal of Eq. 3 by brute force; prior variance is v
+        want = h.vertical - np.einsum("ai,ij,aj->a", Kxs, Kinv, Kxs)
+        assert relerr(p.var, want) <= 1e-11
+        assert np.all(p.var >= 0.0) and np.all(p.var <= h.vertical)
+        np.testing.assert_allclose(p.var, np.diag(p.Sigma), rtol=1e-12, atol=1e-15)
+        # log marginal likelihood: the library's multivariate normal density
+        lml = oracle.log_marginal_likelihood(p.L, y, p.alpha)
+        ref = multivariate_normal(mean=np.zeros(n), cov=K).logpdf(y)
+        assert abs(lml - ref) <= 1e-10 * abs(ref)
+
+
+def test_lml_scaling_law():
+    """(v, s2, y) -> (c v, c s2, sqrt(c) y) leaves the quadratic term unchanged and adds -n/2 log c."""
+    X, y = nfir.nfir_features(5, 48, 4)
+    c = 3.7
+    p1 = oracle.fit(X, y, Hyper(1.0, 1.0, 0.1))
+    p2 = oracle.fit(X, np.sqrt(c) * y, Hyper(1.0, c * 1.0, c * 0.1))
+    l1 = oracle.log_marginal_likelihood(p1.L, y, p1.alpha)
+    l2 = oracle.log_marginal_likelihood(p2.L, np.sqrt(c) * y, p2.alpha)
+    assert abs(l2 - (l1 - 0.5 * 48 * np.log(c))) <= 1e-11 * abs(l1)

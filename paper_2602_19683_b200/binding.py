@@ -228,8 +228,7 @@ def gp_contraction_bench_launch(K: int, reps: int, buf: torch.Tensor) -> float:
     """Enqueue one launch of the contraction steady-state microbenchmark; returns its flop count."""
     f = ctypes.c_double(0.0)
     _check(load().gp_contraction_bench_launch(K, reps, _ptr(buf, torch.uint8), buf.numel(), ctypes.byref(f), None, _stream()),
-           "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
-           "gp_schedule_selfcheck_variance")
+           "gp_contraction_bench_launch")
     return float(f.value)
 
 

@@ -251,3 +251,14 @@ def test_variance_argument_errors(gp):
     with pytest.raises(gp.GpError) as e:
         gp.gp_log_marginal_likelihood(pipe.KL, n, 48, pipe.alpha, pipe.alpha, var)
     assert e.value.code == gp.ERR["TILE"]
+
+
+def test_contraction_bench_launches(gp):
+    """The steady-state contraction microbenchmark bench.py reports runs and counts its flop."""
+    K, reps = 256, 3
+    buf = (torch.rand(gp.gp_contraction_bench_bytes(K, reps) // 8 + 1, dtype=torch.float64, device="cuda") * 1e-3).view(torch.uint8)
+    flop = gp.gp_contraction_bench_launch(K, reps, buf)
+    torch.cuda.synchronize()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    assert flop == sms * reps * 2.0 * 128 * 128 * K
+    assert torch.isfinite(buf.view(torch.float64)[: 3 * K * K]).all()

@@ -167,7 +167,7 @@ int launch_exec_any(int b, const ExecParams& p, int64_t m, int workers, cudaStre
 template <int BLK>
 int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStream_t st) {
     static bool configured = false;
-    constexpr int smem = BLK * (BLK + 1) * 8;
+    constexpr int smem = DiagSmem<BLK>::kBytes;
     if (!configured) {
         if (cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
         configured = true;

@@ -34,6 +34,7 @@
 // CTA's consumers are running (an earlier ticket of the same CTA would be unfinished and lower),
 // all its dependencies are finished, so it completes.
 #pragma once
+#include "gp_diag.cuh"
 #include "gp_gemm.cuh"
 
 namespace gpb {
@@ -88,7 +89,7 @@ struct __align__(16) Job {   // 32 bytes, producer -> consumers
 template <int BLK>
 struct ExecSmem {
     static constexpr int kRing = GemmCfg<BLK>::kRingBytes;
-    static constexpr int kPotrf = BLK * (BLK + 1) * 8;
+    static constexpr int kPotrf = DiagSmem<BLK>::kBytes;
     static constexpr int kWork = kRing > kPotrf ? kRing : kPotrf;       // POTRF factors inside the idle ring
     static constexpr int kFull = kWork;                                  // uint64 full[kStages]
     static constexpr int kEmpty = kFull + 8 * kStages;
@@ -101,85 +102,6 @@ struct ExecSmem {
 
 template <int BLK>
 constexpr int exec_smem_bytes() { return ExecSmem<BLK>::kBytes; }
-
-// ---------------------------------------------------------------------------------------------
-// Diagonal block kernels (shared-memory resident, BLK x BLK, padded stride BLK+1), run by the
-// 256 consumer threads; cbar() is the named barrier among them (the producer warp never joins).
-// POTRF: unblocked right-looking Cholesky of the block; then the inverse of the
-// lower-triangular factor in place, so that TRSM becomes a DMMA product.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cbar() { named_bar_sync<1, kConsumerThreads>(); }
-
-template <int BLK>
-__device__ void chol_lower_smem(double* S, int* d_info, int col0) {
-    constexpr int SP = BLK + 1;
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    for (int j = 0; j < BLK; ++j) {
-        const double d = S[j * SP + j];
-        if (!(d > 0.0) && tid == 0) atomicCAS(d_info, 0, col0 + j + 1);
-        const double ljj = sqrt(d);
-        for (int r = j + 1 + tid; r < BLK; r += kConsumerThreads) S[r * SP + j] = S[r * SP + j] / ljj;
-        cbar();
-        if (tid == 0) S[j * SP + j] = ljj;
-        for (int c = j + 1 + warp; c < BLK; c += kConsumerWarps) {
-            const double lc = S[c * SP + j];
-            for (int r = c + lane; r < BLK; r += 32) S[r * SP + c] = fma(-S[r * SP + j], lc, S[r * SP + c]);
-        }
-        cbar();
-    }
-}
-
-// In-place inverse of the lower-triangular matrix in S (stride BLK+1): from X L = I,
-//   X[j][j] = 1/L[j][j],  X[i][j] = -(sum_{k=j+1..i} X[i][k] L[k][j]) / L[j][j],  j = BLK-1..0.
-// Two threads per row split the sum (even/odd k).
-template <int BLK>
-__device__ void inv_lower_smem(double* S) {
-    constexpr int SP = BLK + 1;
-    const int tid = threadIdx.x;
-    const int i = tid >> 1, half = tid & 1;
-    for (int j = BLK - 1; j >= 0; --j) {
-        double s = 0.0;
-        if (i < BLK && i > j) {
-            for (int k = j + 1 + half; k <= i; k += 2) s = fma(S[i * SP + k], S[k * SP + j], s);
-        }
-        s += __shfl_xor_sync(0xffffffffu, s, 1);
-        const double rd = 1.0 / S[j * SP + j];
-        cbar();
-        if (i < BLK && half == 0) {
-            if (i > j) S[i * SP + j] = -s * rd;
-            else if (i == j) S[j * SP + j] = rd;
-        }
-        cbar();
-    }
-}
-
-template <int BLK>
-__device__ void load_lower_to_smem(double* S, const double* __restrict__ G, int ld) {
-    constexpr int SP = BLK + 1;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
-        const int r = idx / BLK, c = idx % BLK;
-        S[r * SP + c] = (c <= r) ? __ldcg(G + (size_t)r * ld + c) : 0.0;
-    }
-    cbar();
-}
-
-// POTRF job, all consumer threads: G = diagonal block (q,q) of L in global memory (leading
-// dimension t), inv = invD(q).  S is the (idle) operand ring.
-template <int BLK>
-__device__ void potrf_block(double* S, double* __restrict__ G, int t, double* __restrict__ inv, int* d_info, int col0) {
-    constexpr int SP = BLK + 1;
-    load_lower_to_smem<BLK>(S, G, t);
-    chol_lower_smem<BLK>(S, d_info, col0);
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
-        const int r = idx / BLK, c = idx % BLK;
-        if (c <= r) __stcg(G + (size_t)r * t + c, S[r * SP + c]);
-    }
-    inv_lower_smem<BLK>(S);
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
-        const int r = idx / BLK, c = idx % BLK;
-        __stcg(inv + idx, S[r * SP + c]);      // strict upper part of S is still the zeros loaded above
-    }
-}
 
 // ---------------------------------------------------------------------------------------------
 // The producer warp.
@@ -522,17 +444,10 @@ template <int BLK>
 __global__ void __launch_bounds__(kConsumerThreads, 1) trtri_diag_kernel(const double* __restrict__ L, int t, int nbt,
                                                                           double* __restrict__ invD) {
     extern __shared__ __align__(16) double smem[];
-    constexpr int SP = BLK + 1;
     const int q = blockIdx.x;
     const int I = q / nbt;
     const double* G = L + ((size_t)I * (I + 1) / 2 + I) * (size_t)t * t + (size_t)(q % nbt) * BLK * t + (size_t)(q % nbt) * BLK;
-    load_lower_to_smem<BLK>(smem, G, t);
-    inv_lower_smem<BLK>(smem);
-    double* inv = invD + (size_t)q * BLK * BLK;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
-        const int r = idx / BLK, c = idx % BLK;
-        inv[idx] = smem[r * SP + c];
-    }
+    trtri_block<BLK>(smem, G, t, invD + (size_t)q * BLK * BLK);
 }
 
 }  // namespace gpb

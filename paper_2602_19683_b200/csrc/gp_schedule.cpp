@@ -85,7 +85,7 @@ void item_effects(const Shape& s, const SchedItem& it, FW&& wait, FR&& write) {
 struct Cost {
     double per_q, fixed, potrf;
     explicit Cost(int blk) {
-        if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 45.0; }
+        if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 80.0; }
         else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 14.0; }
         else { per_q = 0.8; fixed = 2.5; potrf = 6.0; }
     }

@@ -248,9 +248,21 @@ __device__ void inv_blocked(double* smem) {
 template <int BLK>
 __device__ void load_lower_to_smem(double* S, const double* __restrict__ G, int ld) {
     constexpr int SP = BLK + 1;
-    for (int idx = threadIdx.x; idx < BLK * BLK; idx += kConsumerThreads) {
-        const int r = idx / BLK, c = idx % BLK;
-        S[r * SP + c] = (c <= r) ? __ldcg(G + (size_t)r * ld + c) : 0.0;
+    constexpr int PER = BLK * BLK / kConsumerThreads;    // elements per thread (4, 16 or 64)
+    constexpr int BATCH = PER < 16 ? PER : 16;           // loads in flight per thread
+    for (int b0 = 0; b0 < PER; b0 += BATCH) {
+        double v[BATCH];
+#pragma unroll
+        for (int u = 0; u < BATCH; ++u) {
+            const int idx = (b0 + u) * kConsumerThreads + threadIdx.x;
+            const int r = idx / BLK, c = idx % BLK;
+            v[u] = (c <= r) ? __ldcg(G + (size_t)r * ld + c) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < BATCH; ++u) {
+            const int idx = (b0 + u) * kConsumerThreads + threadIdx.x;
+            S[(idx / BLK) * SP + idx % BLK] = v[u];
+        }
     }
     cbar();
 }

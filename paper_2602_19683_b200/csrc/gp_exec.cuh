@@ -184,8 +184,13 @@ struct Producer {
         mbar_arrive(&job_full[slot]);
         if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
     }
-    __device__ __forceinline__ void stream(const CUtensorMap* mA, int2 a, const CUtensorMap* mB, int2 b, int nk) {
+    // `C`/`ldc` (may be null): the block the consumers will read in their epilogue.  Its rows are pulled into
+    // L2 with cp.async.bulk.prefetch.L2 a few stages before the end of the job -- early enough to hide the
+    // HBM latency, late enough not to be evicted again (at job start, ~140 us earlier, it was).
+    __device__ __forceinline__ void stream(const CUtensorMap* mA, int2 a, const CUtensorMap* mB, int2 b, int nk,
+                                           const double* C = nullptr, int ldc = 0) {
         if (lane != 0) return;
+        const int kpre = nk > kPrefetchLead ? nk - kPrefetchLead : 0;
         for (int kt = 0; kt < nk; ++kt) {
             mbar_wait(&empty[stage], (uint32_t)(phase ^ 1), 2);
             char* dst = ring + (size_t)stage * Cfg::kStageBytes;
@@ -193,11 +198,11 @@ struct Producer {
             tma_load_2d(dst, mA, a.x + kt * kBK, a.y, &full[stage]);
             tma_load_2d(dst + Cfg::kOperandBytes, mB, b.x + kt * kBK, b.y, &full[stage]);
             if (++stage == kStages) { stage = 0; phase ^= 1; }
+            if (kt == kpre && C != nullptr) {
+#pragma unroll 1
+                for (int r = 0; r < BLK; ++r) l2_prefetch_bulk(C + (size_t)r * ldc, BLK * 8);
+            }
         }
-    }
-    // warm L2 with the rows of the C block the consumers will read in their epilogue
-    __device__ __forceinline__ void prefetch_c(const double* C, int ldc) {
-        for (int r = lane; r < BLK; r += 32) l2_prefetch_bulk(C + (size_t)r * ldc, BLK * 8);
     }
 
     // C(gr,gc) -= A(gr,q0:q1) B(gc,q0:q1)^T on (matC, matA, matB) given by op
@@ -229,19 +234,16 @@ struct Producer {
         const int nk = nq * BLK / kBK;
         if (op == OP_UPD_L) {
             double* C = blkL(gr, gc);
-            prefetch_c(C, p.t);
             push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
-            stream(mapL, crdL(gr, q0), mapL, crdL(gc, q0), nk);
+            stream(mapL, crdL(gr, q0), mapL, crdL(gc, q0), nk, C, p.t);
         } else if (op == OP_UPD_V) {
             double* C = blkV(gr, gc);
-            prefetch_c(C, p.t);
             push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
-            stream(mapV, crdV(gr, q0), mapL, crdL(gc, q0), nk);
+            stream(mapV, crdV(gr, q0), mapL, crdL(gc, q0), nk, C, p.t);
         } else {
             double* C = blkS(gr, gc);
-            prefetch_c(C, (int)p.m);
             push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, 0);
-            stream(mapV, crdV(gr, q0), mapV, crdV(gc, q0), nk);
+            stream(mapV, crdV(gr, q0), mapV, crdV(gc, q0), nk, C, (int)p.m);
         }
     }
 

@@ -39,7 +39,7 @@ METRIC = "FP64 tiled Cholesky GFLOP/s and full-cov prediction time at n=32768; %
 # DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant
 # kernel (exec_kernel<128>, the Cholesky DAG) from the ncu --set full capture summarised in
 # profiles/; keyed by (n, tile).  None = not captured for this workload.
-NCU_TRAFFIC_BYTES = {(32768, 1024): 219.6e9}   # profiles/r01c_ncu_step_c3.md (171.2 GB read + 48.4 GB written)
+NCU_TRAFFIC_BYTES = {(32768, 1024): 193.5e9}   # profiles/r01d_ncu_step_c3.md (142.6 GB read + 50.9 GB written)
 
 ORACLE_SAMPLE_BASELINE = (4096, 512)    # (n, m) of the cpu_baseline leg: ~10-30 s of CPU work
 ORACLE_SAMPLE_REFERENCE = (3072, 384)   # per step of --impl reference
@@ -366,6 +366,10 @@ def run_b200(args):
             "ms_per_step": total_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": _config_dict(cfg, tile, args.width, world),
             "cholesky_ms": phase["cholesky"], "cholesky_ms_per_step": per_step_chol,
+            # PAPER.md:163 protocol: mean with a 95 % confidence interval (normal approximation), and the median
+            "cholesky_ms_stats": {"mean": statistics.mean(per_step_chol), "median": statistics.median(per_step_chol),
+                                  "ci95": (1.96 * statistics.stdev(per_step_chol) / len(per_step_chol) ** 0.5) if len(per_step_chol) > 1 else None,
+                                  "runs": len(per_step_chol)},
             "predict_full_cov_ms": phase["solve"] + phase["mean"] + phase["full_cov"],
             "phases_ms": phase, "info": info,
             "pct_fp64_peak": 100.0 * achieved / peak,

@@ -157,8 +157,7 @@ struct Producer {
     __device__ __forceinline__ void poll(const int* addr, int need) {
         if (addr != nullptr && need > 0) {
             const int target = need * kConsumerWarps;
-            unsigned spins = 0;
-            (void)spins;
+            [[maybe_unused]] unsigned spins = 0;
             while (ld_acquire(addr) < target) {
                 GPB_SPIN_GUARD(spins, "dependency poll", target, ld_acquire(addr))
                 __nanosleep(40);

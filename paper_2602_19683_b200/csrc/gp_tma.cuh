@@ -48,8 +48,7 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t by
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0) {
     const uint32_t a = smem_u32(bar);
     uint32_t done;
-    unsigned spins = 0;
-    (void)spins;
+    [[maybe_unused]] unsigned spins = 0;
     (void)tag;
     do {
         GPB_SPIN_GUARD(spins, "mbar_wait", tag, parity)

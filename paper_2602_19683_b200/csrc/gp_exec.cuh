@@ -338,12 +338,8 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
             potrf_block<BLK>(reinterpret_cast<double*>(base), j.C, j.ldc, p.invD + (size_t)j.arg * BLK * BLK, p.d_info, j.arg * BLK);
             fence_proxy_async_global();      // L(q,q), invD(q): read by other CTAs' TMA
             fence_proxy_async_shared();      // the ring is about to be overwritten by TMA again
-            __threadfence();
             cbar();
-            if (threadIdx.x == 0) {
-                __threadfence();
-                atomicAdd(j.sig, kConsumerWarps);
-            }
+            if (threadIdx.x == 0) red_release_add(j.sig, kConsumerWarps);
             continue;
         }
         double acc[Cfg::MI][Cfg::NJ][2];
@@ -370,12 +366,8 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
         }
         store_tile<BLK>(j.C, j.ldc, j.kind, w, acc);
         fence_proxy_async_global();          // this warp's part of C: read by TMA later
-        __threadfence();
         __syncwarp();
-        if (lane == 0) {
-            __threadfence();
-            atomicAdd(j.sig, 1);
-        }
+        if (lane == 0) red_release_add(j.sig, 1);
     }
     if (keeper) {
         unsigned long long* st = p.stats + 8 * (size_t)blockIdx.x;

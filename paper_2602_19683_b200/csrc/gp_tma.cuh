@@ -101,6 +101,14 @@ __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.
 template <int REGS>
 __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(REGS)); }
 
+// Publishing a block version: the barrier (warp or CTA) that precedes it orders the other threads' stores
+// before this thread, and the release makes everything this thread has observed visible at gpu scope
+// before the counter moves -- the pattern of a CUTLASS semaphore release, without the two MEMBAR.SC of
+// __threadfence() + atomicAdd on every job.
+__device__ __forceinline__ void red_release_add(int* p, int v) {
+    asm volatile("red.release.gpu.global.add.s32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+
 __device__ __forceinline__ int ld_acquire(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");

@@ -262,3 +262,30 @@ def test_contraction_bench_launches(gp):
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     assert flop == sms * reps * 2.0 * 128 * 128 * K
     assert torch.isfinite(buf.view(torch.float64)[: 3 * K * K]).all()
+
+
+# ---------------------------------------------------------------- edge cases of the executor and the assembly
+@pytest.mark.parametrize("n,m,D,tile", [
+    (256, 256, 8, 256),       # a single tile: the whole factorisation is one POTRF tile task
+    (2048, 2048, 4, 2048),    # 16 blocks per tile edge: 33 dependency waits per update (more than one per lane)
+    (512, 128, 40, 128),      # D > 32: the assembly stages the features in two chunks
+    (256, 64, 1, 64),         # D = 1
+])
+def test_edge_shapes(gp, n, m, D, tile):
+    X, y = nfir.nfir_features(3 * n + D, n, D)
+    Xs, _ = nfir.nfir_features(5 * m + D, m, D, with_targets=False)
+    h = oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h)
+    out = _run_pipeline(gp, X, y, Xs, h, tile)
+    _check_against_oracle(out, p)
+
+
+def test_single_worker_runs_the_whole_dag(gp):
+    """sched_width = 1: one persistent CTA executes every item in list order (no deadlock, same result)."""
+    n, m, D, tile = 768, 256, 8, 256
+    X, y = nfir.nfir_features(41, n, D)
+    Xs, _ = nfir.nfir_features(42, m, D, with_targets=False)
+    h = oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h)
+    out = _run_pipeline(gp, X, y, Xs, h, tile, width=1)
+    _check_against_oracle(out, p)

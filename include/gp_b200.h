@@ -181,8 +181,8 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
  * to h_stats (host) 8 uint64 per worker CTA:
  *   [0] SM cycles its producer warp spent polling dependency counters,
  *   [1] SM cycles from kernel start to the producer's exit,  [2] work items run,  [3] SM id,
- *   [4]-[7] reserved (0): consumer-side timers were measured with an instrumented build (DESIGN.md
- *   section 5) and then removed -- registers are what limits the consumers' software pipeline;
+ *   [4] SM cycles consumer warp 0 waited for a job descriptor (nothing runnable was handed over),
+ *   [5] reserved,  [6] jobs (GEMM / POTRF block operations) run,  [7] reserved;
  * synchronises the stream.  Returns the number of worker slots copied (<= max_workers) or a
  * negative GP_ERR_*. */
 int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream);

@@ -246,8 +246,8 @@ def gp_schedule_selfcheck_variance(n: int, m: int, tile: int, workers: int = 148
 
 
 def gp_exec_stats(work: torch.Tensor, max_workers: int = 148):
-    """Per-worker (producer_poll_cycles, total_cycles, items, sm_id, 0, 0, 0, 0) of the last executor launch
-    that used `work`."""
+    """Per-worker (producer_poll_cycles, total_cycles, items, sm_id, consumer_job_wait_cycles, 0, jobs, 0) of the
+    last executor launch that used `work`."""
     buf = (ctypes.c_uint64 * (8 * max_workers))()
     w = int(load().gp_exec_stats(_ptr(work, torch.uint8), buf, max_workers, _stream()))
     if w < 0:

@@ -82,7 +82,7 @@ struct __align__(16) Job {   // 32 bytes, producer -> consumers
     int ldc;
     int nk;                // k-stages of kBK
     int kind;
-    int arg;               // POTRF: diagonal block index q
+    int arg;               // POTRF: diagonal block index q; GEMM: versions the job adds to the block (>= 1)
 };
 
 // Shared-memory carve-up (dynamic, base rounded up to 1024 B for the TMA swizzle)
@@ -233,16 +233,29 @@ struct Producer {
         const int nk = nq * BLK / kBK;
         if (op == OP_UPD_L) {
             double* C = blkL(gr, gc);
-            push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
-            stream(mapL, crdL(gr, q0), mapL, crdL(gc, q0), nk, C, p.t);
+            // merged tile columns: one job, one version per column, the panels streamed column by column
+            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
+            push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
+            for (int c = 0; c < ncol; ++c) {
+                const int q = q0 + c * p.nbt;
+                stream(mapL, crdL(gr, q), mapL, crdL(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, p.t);
+            }
         } else if (op == OP_UPD_V) {
             double* C = blkV(gr, gc);
-            push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, 0);
-            stream(mapV, crdV(gr, q0), mapL, crdL(gc, q0), nk, C, p.t);
+            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
+            push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
+            for (int c = 0; c < ncol; ++c) {
+                const int q = q0 + c * p.nbt;
+                stream(mapV, crdV(gr, q), mapL, crdL(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, p.t);
+            }
         } else {
             double* C = blkS(gr, gc);
-            push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, 0);
-            stream(mapV, crdV(gr, q0), mapV, crdV(gc, q0), nk, C, (int)p.m);
+            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
+            push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, ncol);
+            for (int c = 0; c < ncol; ++c) {
+                const int q = q0 + c * p.nbt;
+                stream(mapV, crdV(gr, q), mapV, crdV(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, (int)p.m);
+            }
         }
     }
 
@@ -260,10 +273,10 @@ struct Producer {
         deps_done(t0);
         const int2 d = make_int2(0, gc * BLK);
         if (is_v) {
-            push_job(blkV(gr, gc), p.verV + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 0);
+            push_job(blkV(gr, gc), p.verV + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 1);
             stream(mapV, crdV(gr, gc), mapD, d, BLK / kBK);
         } else {
-            push_job(blkL(gr, gc), p.verL + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 0);
+            push_job(blkL(gr, gc), p.verL + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 1);
             stream(mapL, crdL(gr, gc), mapD, d, BLK / kBK);
         }
     }
@@ -319,18 +332,20 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
     w.init(warp, lane);
     int stage = 0, phase = 0, slot = 0, jphase = 0;
     int pending = -1;                      // ring stage consumed but not yet released
-    bool ready = false;                    // the stage at (stage, phase) is already known to be full
+    const bool keeper = (threadIdx.x == 0) && p.stats != nullptr;     // consumer-side statistics
+    long long job_wait = 0;
+    unsigned int njobs = 0;
     for (;;) {
+        const long long tj = clock64();
         mbar_wait(&job_full[slot], (uint32_t)jphase, 3);
-        // Only nk and kind stay in registers through the main loop; C, sig and ldc are read again from the
-        // descriptor for the epilogue, and the slot is handed back after that (registers are what limits
-        // the software pipeline below, the 4-slot queue is not).
-        const int cur = slot;
-        const int nk = jobs[cur].nk, kind = jobs[cur].kind;
+        if (keeper) job_wait += clock64() - tj;
+        const Job j = jobs[slot];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&job_empty[slot]);
         if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
-        if (kind == JOB_EXIT) break;
-        if (kind == JOB_POTRF) {
-            const Job j = jobs[cur];
+        if (j.kind == JOB_EXIT) break;
+        ++njobs;
+        if (j.kind == JOB_POTRF) {
             // every earlier stage has been consumed by this warp; the barrier inside makes that true for all warps
             cbar();
             potrf_block<BLK>(reinterpret_cast<double*>(base), j.C, j.ldc, p.invD + (size_t)j.arg * BLK * BLK, p.d_info, j.arg * BLK);
@@ -338,7 +353,6 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
             fence_proxy_async_shared();      // the ring is about to be overwritten by TMA again
             cbar();
             if (threadIdx.x == 0) red_release_add(j.sig, kConsumerWarps);
-            if (lane == 0) mbar_arrive(&job_empty[cur]);
             continue;
         }
         double acc[Cfg::MI][Cfg::NJ][2];
@@ -346,55 +360,33 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
         for (int i = 0; i < Cfg::MI; ++i)
 #pragma unroll
             for (int jj = 0; jj < Cfg::NJ; ++jj) acc[i][jj][0] = acc[i][jj][1] = 0.0;
-        // Main loop, software-pipelined ACROSS stage boundaries: the fragments of k-step 0 of stage s+1 are
-        // loaded before the DMMAs of k-step 3 of stage s issue, so the tensor pipe does not drain at a
-        // boundary (both warps of a sub-partition reach it together: without this ~100 cycles of every
-        // ~4000 were lost to the wait, the address arithmetic and the first LDS latency).  Whether stage s+1
-        // has landed is probed (non-blocking) at the top of stage s; only a negative answer costs a wait.
-        Frags<BLK> f0, f1;
-        if (!ready) mbar_wait(&full[stage], (uint32_t)phase, 4);
-        load_frags<BLK>(base + (size_t)stage * Cfg::kStageBytes, 0, w, f0);
-        for (int kt = 0; kt < nk; ++kt) {
-            const char* cs = base + (size_t)stage * Cfg::kStageBytes;
-            const int ns = (stage + 1 == kStages) ? 0 : stage + 1;
-            const int np = (stage + 1 == kStages) ? phase ^ 1 : phase;
-            ready = mbar_test(&full[ns], (uint32_t)np);
-            // Deferred release: the stage consumed in the previous iteration is handed back only now.
-            // Releasing a stage right behind its last LDS.64 is NOT safe: the arrive does not wait for
-            // loads still in flight and the TMA refill then races them (measured: 11 of 80 runs of
-            // config 2 wrong at 1e-5; 0 of 80 with a fence.acq_rel.cta before the arrive or with the
-            // deferral).  The last loads of the released stage were issued before the 2 x MI x NJ DMMAs
-            // that end the previous iteration, on the other side of the loop edge.  `pending` carries
-            // across jobs; a stage still pending at a POTRF or at EXIT is not needed by anyone.
+        for (int kt = 0; kt < j.nk; ++kt) {
+            mbar_wait(&full[stage], (uint32_t)phase, 4);
+            // Deferred release: the stage consumed one step ago is handed back only now.  Releasing a
+            // stage right behind its last LDS.64 is NOT safe -- the arrive does not wait for loads
+            // still in flight and the TMA refill then races them (measured: 11 of 80 runs of config 2
+            // came out wrong at 1e-5; 0 of 80 with either a fence.acq_rel.cta before the arrive or
+            // this deferral, which costs nothing but one stage of ring depth).  By now every DMMA of
+            // the previous stage has issued, so every load of it has returned.  `pending` carries
+            // across jobs; a stage still pending at a POTRF or at EXIT is simply not needed.
             if (pending >= 0) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[pending]);
             }
             pending = stage;
-            load_frags<BLK>(cs, 1, w, f1);
-            mma_frags<BLK>(acc, f0);
-            load_frags<BLK>(cs, 2, w, f0);
-            mma_frags<BLK>(acc, f1);
-            load_frags<BLK>(cs, 3, w, f1);
-            mma_frags<BLK>(acc, f0);
-            if (kt + 1 < nk) {
-                if (!ready) mbar_wait(&full[ns], (uint32_t)np, 4);
-                load_frags<BLK>(base + (size_t)ns * Cfg::kStageBytes, 0, w, f0);
-            }
-            mma_frags<BLK>(acc, f1);
-            stage = ns;
-            phase = np;
+            consume_stage<BLK>(base + (size_t)stage * Cfg::kStageBytes, w, acc);
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        {
-            const Job j = jobs[cur];
-            store_tile<BLK>(j.C, j.ldc, kind, w, acc);
-            fence_proxy_async_global();          // this warp's part of C: read by TMA later
-            __syncwarp();
-            if (lane == 0) {
-                red_release_add(j.sig, 1);
-                mbar_arrive(&job_empty[cur]);
-            }
-        }
+        store_tile<BLK>(j.C, j.ldc, j.kind, w, acc);
+        fence_proxy_async_global();          // this warp's part of C: read by TMA later
+        __syncwarp();
+        if (lane == 0) red_release_add(j.sig, j.arg);   // versions this job adds (tile columns it covered)
+    }
+    if (keeper) {
+        unsigned long long* st = p.stats + 8 * (size_t)blockIdx.x;
+        st[4] = (unsigned long long)job_wait;
+        st[5] = 0;
+        st[6] = (unsigned long long)njobs;
     }
 }
 
@@ -446,7 +438,6 @@ exec_kernel(const __grid_constant__ ExecParams p, const __grid_constant__ CUtens
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         unsigned long long* st = p.stats + 8 * (size_t)blockIdx.x;
         st[0] = (unsigned long long)prod.poll_cycles;
-        st[4] = st[5] = st[6] = st[7] = 0;
         st[1] = (unsigned long long)(clock64() - t_start);
         st[2] = nrun;
         st[3] = smid;

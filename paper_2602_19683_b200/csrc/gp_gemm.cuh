@@ -98,37 +98,32 @@ struct WarpTile {
     }
 };
 
-// Fragments of one k-step (4 deep) of the warp's (MI*8) x (NJ*8) product.
+// One k-stage (16 deep) of the warp's (MI*8) x (NJ*8) product out of a filled ring slot.
 template <int BLK>
-struct Frags {
-    double a[GemmCfg<BLK>::MI], b[GemmCfg<BLK>::NJ];
-};
-
-// LDS.64 of k-step ks (0..3) of a filled ring slot.
-template <int BLK>
-__device__ __forceinline__ void load_frags(const char* stage, int ks, const WarpTile<BLK>& w, Frags<BLK>& f) {
+__device__ __forceinline__ void consume_stage(const char* stage, const WarpTile<BLK>& w,
+                                              double (&acc)[GemmCfg<BLK>::MI][GemmCfg<BLK>::NJ][2]) {
     using Cfg = GemmCfg<BLK>;
     const char* sA = stage;
     const char* sB = stage + Cfg::kOperandBytes;
-    // k = 4*ks + t lives in chunk (2*ks + t/2) ^ (row & 7): the ks part is an XOR of bits 5-6
-    const uint32_t a0 = w.a_off[0] ^ (uint32_t)(ks << 5), a1 = w.a_off[1] ^ (uint32_t)(ks << 5);
-    const uint32_t b0 = w.b_off[0] ^ (uint32_t)(ks << 5), b1 = w.b_off[1] ^ (uint32_t)(ks << 5);
 #pragma unroll
-    for (int i = 0; i < Cfg::MI; ++i) f.a[i] = *reinterpret_cast<const double*>(sA + ((i & 1) ? a1 : a0) + (i >> 1) * 16 * 128);
+    for (int ks = 0; ks < kBK / 4; ++ks) {
+        double a[Cfg::MI], b[Cfg::NJ];
+        // k = 4*ks + t lives in chunk (2*ks + t/2) ^ (row & 7): the ks part is an XOR of bits 5-6
+        const uint32_t a0 = w.a_off[0] ^ (uint32_t)(ks << 5), a1 = w.a_off[1] ^ (uint32_t)(ks << 5);
+        const uint32_t b0 = w.b_off[0] ^ (uint32_t)(ks << 5), b1 = w.b_off[1] ^ (uint32_t)(ks << 5);
 #pragma unroll
-    for (int j = 0; j < Cfg::NJ; ++j) {
-        if (Cfg::NJ % 2 == 0) f.b[j] = *reinterpret_cast<const double*>(sB + ((j & 1) ? b1 : b0) + (j >> 1) * 16 * 128);
-        else f.b[j] = *reinterpret_cast<const double*>(sB + b0 + j * 8 * 128);
+        for (int i = 0; i < Cfg::MI; ++i)
+            a[i] = *reinterpret_cast<const double*>(sA + ((i & 1) ? a1 : a0) + (i >> 1) * 16 * 128);
+#pragma unroll
+        for (int j = 0; j < Cfg::NJ; ++j) {
+            if (Cfg::NJ % 2 == 0) b[j] = *reinterpret_cast<const double*>(sB + ((j & 1) ? b1 : b0) + (j >> 1) * 16 * 128);
+            else b[j] = *reinterpret_cast<const double*>(sB + b0 + j * 8 * 128);
+        }
+#pragma unroll
+        for (int i = 0; i < Cfg::MI; ++i)
+#pragma unroll
+            for (int j = 0; j < Cfg::NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
     }
-}
-
-template <int BLK>
-__device__ __forceinline__ void mma_frags(double (&acc)[GemmCfg<BLK>::MI][GemmCfg<BLK>::NJ][2], const Frags<BLK>& f) {
-    using Cfg = GemmCfg<BLK>;
-#pragma unroll
-    for (int i = 0; i < Cfg::MI; ++i)
-#pragma unroll
-        for (int j = 0; j < Cfg::NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], f.a[i], f.b[j]);
 }
 
 // Epilogue of one warp: C <- C - acc (kSub) or C <- acc (kSet).  Lane (g,t) of accumulator block

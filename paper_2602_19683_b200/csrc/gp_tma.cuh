@@ -64,21 +64,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
     } while (!done);
 }
 
-// non-blocking probe of the same condition (used to learn early that the NEXT stage is already there)
-__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
-    uint32_t done;
-    asm volatile(
-        "{\n"
-        " .reg .pred p;\n"
-        " mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        " selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return done != 0;
-}
-
 // ---- TMA ----------------------------------------------------------------------------------------
 // 2-D tiled load global -> shared, completion counted in bytes on `bar`.  c0 = inner (contiguous)
 // coordinate, c1 = outer coordinate, both in elements of the tensor map.

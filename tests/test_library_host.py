@@ -67,7 +67,8 @@ def test_task_counts_match_paper_dag(gp):
     for M, want in ((4, 20), (8, 120), (16, 816), (32, 5984)):
         tasks, items = gp.gp_cholesky_task_counts(M * 128, 128)
         assert tasks == want
-        assert items >= tasks
+        # a work item is a block-level piece of a tile task or (trailing updates) of up to 4 merged tile tasks
+        assert items > 0 and 4 * items >= tasks
 
 
 @pytest.mark.parametrize("n,m,tile", [

@@ -39,7 +39,7 @@ METRIC = "FP64 tiled Cholesky GFLOP/s and full-cov prediction time at n=32768; %
 # DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant
 # kernel (exec_kernel<128>, the Cholesky DAG) from the ncu --set full capture summarised in
 # profiles/; keyed by (n, tile).  None = not captured for this workload.
-NCU_TRAFFIC_BYTES = {(32768, 1024): 193.5e9}   # profiles/r01d_ncu_step_c3.md (142.6 GB read + 50.9 GB written)
+NCU_TRAFFIC_BYTES = {(32768, 1024): 148.8e9}   # profiles/r01e_ncu_step_c3.md (124.6 GB read + 24.2 GB written)
 
 ORACLE_SAMPLE_BASELINE = (4096, 512)    # (n, m) of the cpu_baseline leg: ~10-30 s of CPU work
 ORACLE_SAMPLE_REFERENCE = (3072, 384)   # per step of --impl reference

@@ -82,7 +82,8 @@ int gp_assemble_tiles(const double* dA, int64_t na, const double* dB, int64_t nb
  *        terminate and dKL is unspecified.
  *   dWork/work_bytes: scratch, at least the `chol` size from gp_workspace_bytes(). On exit it
  *        holds the inverted diagonal blocks of L that gp_predict_full_cov recomputes for itself,
- *        so it may be freed or reused immediately. */
+ *        so it may be freed or reused immediately.
+ *   Limits: n <= 2^22 and n / gp_block_size(tile) <= 65535 (GP_ERR_SIZE otherwise). */
 int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork,
                       size_t work_bytes, void* stream);
 

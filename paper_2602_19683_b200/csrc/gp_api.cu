@@ -335,6 +335,7 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
     const int b = pick_block(tile);
+    if (n / b > 65535) return GP_ERR_SIZE;            // block indices travel in 16 bits of a work item
     const CholWs w = chol_ws(n, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -413,6 +414,7 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     if (rc != GP_OK) return rc;
     if (!hyper_ok(h)) return GP_ERR_HYPER;
     const int b = pick_block(tile);
+    if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;   // block indices travel in 16 bits of a work item
     const CovWs w = cov_ws(n, m, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;

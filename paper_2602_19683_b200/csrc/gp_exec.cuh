@@ -20,8 +20,9 @@
 //
 // Work items are block-level (b x b, b = 128 for tiles that are multiples of 128) pieces of the
 // paper's tile tasks (readings A3/A4):
-//   UPD   C(gr,gc) -= sum_{q in [q0,q1)} A(gr,q) B(gc,q)^T      SYRK / GEMM tiles (q-range = one
-//                                                                tile column J), POTRF sub-updates
+//   UPD   C(gr,gc) -= sum_{q in [q0,q1)} A(gr,q) B(gc,q)^T      SYRK / GEMM tiles (q-range = one to four
+//                                                                consecutive tile columns, one version
+//                                                                each), POTRF sub-updates
 //   TRSM  C(gr,gc)  = C(gr,gc) invD(gc)^T                        panel solve with the inverted
 //                                                                diagonal block
 //   POTRF L(q,q)    = chol(C(q,q)), invD(q) = L(q,q)^-1          diagonal block

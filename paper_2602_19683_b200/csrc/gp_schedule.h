@@ -7,6 +7,10 @@
 // priority, per-item cost model) decides the order in which items are handed out.  The order is
 // a topological order of the DAG by construction, which is what makes the in-order ticket
 // scheme deadlock-free; the simulated timing only has to be roughly right for waits to be short.
+// Trailing updates of up to four consecutive tile columns are merged into one item per block
+// (environment variable GP_B200_MERGE_COLUMNS = 1..4, default 4, read when the first schedule is built);
+// the priority of an item is the critical-path length of its tile task, so that the items in flight
+// share operand panels in L2.
 #pragma once
 #include <cstdint>
 #include <vector>

@@ -36,13 +36,17 @@ if ROOT not in sys.path:
 
 METRIC = "FP64 tiled Cholesky GFLOP/s and full-cov prediction time at n=32768; % FP64 peak"
 
-# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant
-# kernel (exec_kernel<128>, the Cholesky DAG) from the ncu --set full capture summarised in
-# profiles/; keyed by (n, tile).  None = not captured for this workload.
-NCU_TRAFFIC_BYTES = {(32768, 1024): 148.8e9}   # profiles/r01e_ncu_step_c3.md (124.6 GB read + 24.2 GB written)
+# DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel
+# (exec_kernel<128>, the Cholesky DAG) comes from the ncu --set full captures summarised under
+# profiles/: profiles/ncu_traffic.json records, per (n, tile), the bytes, the capture it came from, the
+# commit and the fingerprint of the work-item schedule it was taken with.  bench.py reports the
+# figure only while the library still builds the same schedule, else null.
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 
-ORACLE_SAMPLE_BASELINE = (4096, 512)    # (n, m) of the cpu_baseline leg: ~10-30 s of CPU work
-ORACLE_SAMPLE_REFERENCE = (3072, 384)   # per step of --impl reference
+ORACLE_SAMPLE = (4096, 512)             # (n, m) of the sampled oracle pipeline pass (configs 3-4) and of --impl reference
+ORACLE_CHOLESKY_SIZES = (4096, 8192)    # measured unblocked-Cholesky passes the n^3 extrapolation starts from (configs 3-4)
+ORACLE_CHOLESKY_SIZES_LONG = (4096, 8192, 16384)   # with --cpu-baseline-long (minutes of CPU)
+E2E_UNIT = "GFLOP/s"                    # identical in both arms, so that the driver can form e2e_ratio
 
 
 def _parse():
@@ -55,6 +59,8 @@ def _parse():
     ap.add_argument("--tile", type=int, default=0, help="override the config's tile size")
     ap.add_argument("--width", type=int, default=0, help="scheduler width (persistent CTAs), 0 = one per SM")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-long", action="store_true",
+                    help="configs 3-4: also time the oracle's Cholesky at n=16384; config 2: also the 1-thread full pass")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--cusolver-ref", action="store_true")
     return ap.parse_args()
@@ -158,8 +164,9 @@ def _config_dict(cfg, tile, width, world):
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_run(n, m, D, cfg, seed_shift=0):
-    """One oracle pass (a1-a12) on an (n, m) sample of the workload; returns per-phase seconds."""
+def oracle_run(n, m, D, cfg, seed_shift=0, cholesky_only=False):
+    """One oracle pass (a1-a12, or a1-a6 with cholesky_only) on an (n, m) sample of the workload's
+    generator; returns per-phase seconds."""
     import oracle
     from paper_2602_19683_b200 import nfir
     X, y = nfir.nfir_features(1000 + cfg.index + seed_shift, n, D)
@@ -170,6 +177,8 @@ def oracle_run(n, m, D, cfg, seed_shift=0):
     t1 = time.perf_counter()
     L = oracle.cholesky(K)
     t2 = time.perf_counter()
+    if cholesky_only:
+        return {"assemble_s": t1 - t0, "cholesky_s": t2 - t1, "predict_s": None, "total_s": t2 - t0}
     beta = oracle.forward_subst(L, y)
     alpha = oracle.backward_subst(L, beta)
     fitted = oracle.Prediction(K=None, L=L, beta=beta, alpha=alpha)
@@ -178,15 +187,59 @@ def oracle_run(n, m, D, cfg, seed_shift=0):
     return {"assemble_s": t1 - t0, "cholesky_s": t2 - t1, "predict_s": t3 - t2, "total_s": t3 - t0}
 
 
-def cpu_baseline(cfg):
+def cpu_baseline(cfg, long_run=False):
+    """The oracle as it stands on the box's host cores.
+    Configs 0-2: the FULL oracle on the same config, all threads, and a 1-thread time beside it (config 2:
+    the 1-thread pass only with --cpu-baseline-long: it is minutes).  Configs 3-4: the full oracle would run
+    for many minutes, so the Cholesky is MEASURED at n = 4096 and 8192 (16384 too with --cpu-baseline-long)
+    and the figure for the config's own n is the n^3 scaling of the largest measured pass, under the key
+    `extrapolated` (optimistic for the CPU: the unblocked oracle is memory-bound and slows down with n);
+    the prediction phase is measured on an (n=4096, m=512) sample."""
     import oracle
-    n, m = ORACLE_SAMPLE_BASELINE
-    n, m = min(n, cfg.n), min(m, cfg.m)
-    r = oracle_run(n, m, cfg.D, cfg)
-    return {"value": n ** 3 / 3.0 / r["cholesky_s"] / 1e9, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"one oracle pass on n={n}, m={m}, D={cfg.D} of the same generator (unblocked Cholesky {r['cholesky_s']:.2f} s, "
-                      f"whole pipeline {r['total_s']:.2f} s)",
-            "predict_full_cov_ms": r["predict_s"] * 1e3, "cholesky_ms": r["cholesky_s"] * 1e3}
+    threads = oracle.num_threads()
+    flop = lambda n: n ** 3 / 3.0
+    if cfg.index <= 2:
+        r = oracle_run(cfg.n, cfg.m, cfg.D, cfg)
+        out = {"value": flop(cfg.n) / r["cholesky_s"] / 1e9, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+               "sample": f"the full oracle on the same config (n={cfg.n}, m={cfg.m}, D={cfg.D}), one pass, {threads} threads",
+               "cholesky_ms": r["cholesky_s"] * 1e3, "predict_full_cov_ms": r["predict_s"] * 1e3, "pipeline_ms": r["total_s"] * 1e3}
+        if cfg.index < 2 or long_run:
+            oracle.set_num_threads(1)
+            try:
+                r1 = oracle_run(cfg.n, cfg.m, cfg.D, cfg)
+            finally:
+                oracle.set_num_threads(threads)
+            out["one_thread"] = {"value": flop(cfg.n) / r1["cholesky_s"] / 1e9, "cholesky_ms": r1["cholesky_s"] * 1e3,
+                                 "predict_full_cov_ms": r1["predict_s"] * 1e3, "pipeline_ms": r1["total_s"] * 1e3}
+        else:
+            out["one_thread"] = None      # run with --cpu-baseline-long
+        return out
+    sizes = ORACLE_CHOLESKY_SIZES_LONG if long_run else ORACLE_CHOLESKY_SIZES
+    measured = []
+    for n in sizes:
+        r = oracle_run(n, 32, cfg.D, cfg, cholesky_only=True)
+        measured.append({"n": n, "cholesky_s": r["cholesky_s"], "gflops": flop(n) / r["cholesky_s"] / 1e9})
+    ns, ms = ORACLE_SAMPLE
+    rp = oracle_run(ns, ms, cfg.D, cfg)
+    last = measured[-1]
+    ext_s = last["cholesky_s"] * (cfg.n / last["n"]) ** 3
+    return {"value": last["gflops"], "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+            "sample": f"unblocked oracle Cholesky MEASURED at n={', '.join(str(x['n']) for x in measured)} (D={cfg.D}, same generator, "
+                      f"{threads} threads); value = the rate of the largest measured pass; the figure for n={cfg.n} is extrapolated",
+            "measured": measured,
+            "extrapolated": {"n": cfg.n, "cholesky_s": ext_s, "gflops": flop(cfg.n) / ext_s / 1e9,
+                             "how": f"t(n) = t({last['n']}) * (n/{last['n']})^3: flop scaling only, optimistic for the CPU "
+                                    "(the unblocked oracle is memory-bound and its rate falls as n grows)"},
+            "pipeline_sample": {"n": ns, "m": ms, "cholesky_ms": rp["cholesky_s"] * 1e3, "predict_full_cov_ms": rp["predict_s"] * 1e3,
+                                "pipeline_ms": rp["total_s"] * 1e3}}
+
+
+def reference_sample(cfg):
+    """(n, m) one step of --impl reference runs: the config itself where the oracle finishes it in seconds
+    (configs 0-1), otherwise a bounded sample of the same generator."""
+    if cfg.index <= 1:
+        return cfg.n, cfg.m, False
+    return min(ORACLE_SAMPLE[0], cfg.n), min(ORACLE_SAMPLE[1], cfg.m), True
 
 
 def run_reference(args):
@@ -195,8 +248,7 @@ def run_reference(args):
         return 0
     import oracle
     cfg, tile = _config(args)
-    n, m = ORACLE_SAMPLE_REFERENCE
-    n, m = min(n, cfg.n), min(m, cfg.m)
+    n, m, sampled = reference_sample(cfg)
     for _ in range(args.warmup):
         oracle_run(n, m, cfg.D, cfg)
     chol, total, pred = 0.0, 0.0, 0.0
@@ -204,15 +256,39 @@ def run_reference(args):
         r = oracle_run(n, m, cfg.D, cfg)
         chol += r["cholesky_s"]; total += r["total_s"]; pred += r["predict_s"]
     value = args.steps * (n ** 3 / 3.0) / chol / 1e9
-    sample = f"each step = one oracle pass on n={n}, m={m}, D={cfg.D} of the same generator"
+    sample = (f"each step = one oracle pass (a1-a12) on an n={n}, m={m}, D={cfg.D} SAMPLE of the same generator" if sampled
+              else f"each step = one oracle pass (a1-a12) on the config itself (n={n}, m={m}, D={cfg.D})")
+    config = _config_dict(cfg, tile, args.width, world)
+    if sampled:     # say what was actually run: the oracle cannot finish this config within the driver's time
+        config["workload"] = (f"SAMPLE n={n} m={m} D={cfg.D} of " + config["workload"] +
+                              " -- the unblocked CPU oracle runs a bounded sample, not the config")
+        config["sample_n"], config["sample_m"] = n, m
+    e2e_value = args.steps * (n ** 3 / 3.0) / total / 1e9     # same definition as the b200 arm: n^3/3 over the whole pipeline time
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": _config_dict(cfg, tile, args.width, world),
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
             "predict_full_cov_ms": pred / args.steps * 1e3, "gpu_launches": 0,
             "cpu_baseline": {"value": value, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
-            "e2e": {"value": value, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+            "e2e": {"value": e2e_value, "unit": E2E_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "definition": "n^3/3 of the problem actually run over its whole pipeline time (a1-a12)"}}
     print(json.dumps(line), flush=True)
     return 0
+
+
+def ncu_traffic(gp, n, tile):
+    """DRAM bytes of one Cholesky launch from profiles/ncu_traffic.json, or None when there is no capture for
+    this workload or the library no longer builds the schedule the capture was taken with."""
+    try:
+        table = json.load(open(NCU_TRAFFIC_FILE))
+    except (OSError, ValueError):
+        return None, "no profiles/ncu_traffic.json"
+    rec = table.get(f"n={n},tile={tile}")
+    if rec is None:
+        return None, "no ncu capture for this workload"
+    fp = "%016x" % gp.gp_schedule_fingerprint(n, 0, tile, 148)
+    if rec.get("schedule_fingerprint") != fp:
+        return None, f"stale: captured with schedule {rec.get('schedule_fingerprint')} at {rec.get('commit')}, this build makes {fp}"
+    return float(rec["dram_bytes"]), f"{rec.get('source')} (commit {rec.get('commit')})"
 
 
 # ------------------------------------------------------------------------------------------------
@@ -276,6 +352,9 @@ def run_b200(args):
     Xs, _ = nfir.nfir_features(seed_test, m, D, with_targets=False)
     hX, hY, hXs = (torch.from_numpy(a).pin_memory() for a in (X, y, Xs))
     dX, dY, dXs = hX.cuda(), hY.cuda(), hXs.cuda()
+    # step a6, host half: build + upload the static schedules once, outside every timed region (the first
+    # compute call for a shape would otherwise do it, blocking the host; include/gp_b200.h)
+    schedule_build_ms = gp.gp_prepare(n, m, tile, gp.GP_PREPARE_CHOLESKY | gp.GP_PREPARE_FULL_COV | gp.GP_PREPARE_VARIANCE)
     pipe = gp.GpPipeline(n, m, D, tile, h, sched_width=args.width)
 
     def barrier():
@@ -309,6 +388,18 @@ def run_b200(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     info = int(pipe.info.item())
+    # cheap parity guard on the LAST timed step's outputs (full parity is tests/test_gpu_full_size.py):
+    # ||L (L^T z) - K z|| / ||K z|| with K z = sum_j k(x_i, x_j) z_j + noise z_i from the library's own fused
+    # kernel-matrix product (gp_predict_mean) and L unpacked by gp_tiles_to_dense; torch only does the two
+    # triangular matrix-vector products of the check itself, outside every timed region.
+    z = torch.randn(n, dtype=torch.float64, device="cuda", generator=torch.Generator(device="cuda").manual_seed(5))
+    Kz = torch.empty(n, dtype=torch.float64, device="cuda")
+    gp.gp_predict_mean(dX, z, dX, h, Kz)
+    Kz += cfg.noise * z
+    Ld = pipe.dense_L()
+    resid = float((torch.mv(Ld, torch.mv(Ld.t(), z)) - Kz).norm() / Kz.norm())
+    del Ld, Kz, z
+    torch.cuda.empty_cache()
     phase = {nm: sum(events[s][i].elapsed_time(events[s][i + 1]) for s in range(args.steps)) for i, nm in enumerate(names)}
     total_ms = sum(events[s][0].elapsed_time(events[s][5]) for s in range(args.steps))
     per_step_chol = [events[s][1].elapsed_time(events[s][2]) for s in range(args.steps)]
@@ -356,7 +447,7 @@ def run_b200(args):
         peaks = measure_fp64_peak(gp, torch)
         peak = peaks["dmma_sustained_tflops"]
         achieved = flop / (phase["cholesky"] * 1e-3) / 1e12
-        traffic = NCU_TRAFFIC_BYTES.get((n, tile))
+        traffic, traffic_source = ncu_traffic(gp, n, tile)
         try:
             mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         except OSError:
@@ -371,14 +462,16 @@ def run_b200(args):
                                   "ci95": (1.96 * statistics.stdev(per_step_chol) / len(per_step_chol) ** 0.5) if len(per_step_chol) > 1 else None,
                                   "runs": len(per_step_chol)},
             "predict_full_cov_ms": phase["solve"] + phase["mean"] + phase["full_cov"],
-            "phases_ms": phase, "info": info,
+            "phases_ms": phase, "info": info, "residual_LLt_vs_K_last_step": resid,
+            "schedule_build_ms": schedule_build_ms,
             "pct_fp64_peak": 100.0 * achieved / peak,
-            "e2e": {"value": world * flop / (e2e_ms * 1e-3) / 1e9, "unit": "GFLOP/s (n^3/3 over the whole host-to-host pipeline time)",
-                    "ms": e2e_ms, "h2d_bytes_per_step": (n * D + n + m * D) * 8, "d2h_bytes_per_step": (m + m * m) * 8 + 4,
+            "e2e": {"value": world * flop / (e2e_ms * 1e-3) / 1e9, "unit": E2E_UNIT,
+                    "definition": "n^3/3 over the whole host-to-host pipeline time (a1-a12 + copies)", "ms": e2e_ms, "h2d_bytes_per_step": (n * D + n + m * D) * 8, "d2h_bytes_per_step": (m + m * m) * 8 + 4,
                     "info": info_e2e, "call": "gp_pipeline_host (pinned host buffers)"},
             "gpu_launches": sum(LAUNCHES_PER_STEP.values()) * args.steps,
             "roofline": {"bound": "tensor", "kernel": "exec_kernel<128> (tiled Cholesky DAG: POTRF/TRSM/SYRK/GEMM; TMA-fed FP64 DMMA)",
-                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
+                         "compulsory_bytes": (n // tile) * (n // tile + 1) * tile * tile * 8,   # read K once + write L once
                          "peak_source": "gp_fp64_peak_launch DMMA.8x8x4 register-resident microbenchmark, measured live, "
                                         "sustained ~2 s loop (kernel is timed inside a long step)",
                          "peak_burst": peaks["dmma_burst_tflops"], "dfma_burst": peaks["dfma_burst_tflops"],
@@ -392,7 +485,7 @@ def run_b200(args):
             "next_rows": next_rows,
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg)
+            line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_baseline_long)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -402,7 +495,9 @@ def run_b200(args):
 
 # ------------------------------------------------------------------------------------------------
 def run_sweep(args):
-    """Config 2: tile in {256,512,1024} x scheduler width in {1,2,4,8,auto}; Cholesky + full-cov."""
+    """Config 2: tile in {256,512,1024} x scheduler width in {1,2,4,8,16,32,64,148}; Cholesky + full-cov
+    (the analogue of the paper's stream-count x tile-count sweep, Fig. 3).
+    protocol: mean of the repetitions with a 95 % confidence interval (at least 5 repetitions; 10 from width 8)."""
     import torch
     from paper_2602_19683_b200 import binding as gp, nfir
     cfg = nfir.CONFIGS[2]
@@ -410,11 +505,17 @@ def run_sweep(args):
     X, y, Xs = nfir.make_inputs(cfg)
     dX, dY, dXs = (torch.from_numpy(a).cuda() for a in (X, y, Xs))
     h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
     rows = []
+
+    def ci95(v):
+        return 1.96 * statistics.stdev(v) / len(v) ** 0.5 if len(v) > 1 else None
+
     for tile in (256, 512, 1024):
-        for width in (1, 2, 4, 8, 0):
+        gp.gp_prepare(n, m, tile)
+        for width in (1, 2, 4, 8, 16, 32, 64, sms):
             pipe = gp.GpPipeline(n, m, D, tile, h, sched_width=width)
-            reps = 2 if width in (1, 2) else 5
+            reps = 5 if width < 8 else 10
             tc, tp = [], []
             for r in range(reps + 1):
                 pipe.assemble(dX)
@@ -424,8 +525,9 @@ def run_sweep(args):
                 torch.cuda.synchronize()
                 if r > 0:
                     tc.append(e[0].elapsed_time(e[1])); tp.append(e[1].elapsed_time(e[2]))
-            rows.append({"tile": tile, "sched_width": width or "auto", "cholesky_ms": statistics.mean(tc),
-                         "cholesky_gflops": n ** 3 / 3.0 / (statistics.mean(tc) * 1e-3) / 1e9, "predict_full_cov_ms": statistics.mean(tp)})
+            rows.append({"tile": tile, "sched_width": width, "reps": reps, "cholesky_ms": statistics.mean(tc), "cholesky_ms_ci95": ci95(tc),
+                         "cholesky_gflops": n ** 3 / 3.0 / (statistics.mean(tc) * 1e-3) / 1e9,
+                         "predict_full_cov_ms": statistics.mean(tp), "predict_full_cov_ms_ci95": ci95(tp)})
             del pipe
     print(json.dumps({"sweep": "c2 n=8192 m=1024 D=8: tile x scheduler width (PAPER.md:169 analogue)", "rows": rows}), flush=True)
     return 0

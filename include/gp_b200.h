@@ -7,10 +7,17 @@
  * Conventions for every entry point
  *   - All `d*` pointers are DEVICE pointers to FP64 (or int where stated), 16-byte aligned,
  *     owned by the caller.  The library never frees or keeps caller memory.  Its only state is
- *     a lazily built per-process cache of device-resident task schedules (a few MB, keyed by
- *     problem shape) that gp_release_cached_schedules() drops.
+ *     a per-process cache of device-resident task schedules (16 bytes per work item: 2.4 MB for
+ *     the n = 32768 / tile 1024 factorisation, 9.4 MB for n = 65536 / tile 2048), keyed by
+ *     (device, kind, n/tile, m/tile, tile/block, block); it never evicts, and
+ *     gp_release_cached_schedules() drops it.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every
- *     call is stream-ordered and does not synchronise the host.
+ *     call is stream-ordered and does not synchronise the host, with ONE exception: the first
+ *     gp_cholesky_tiled / gp_predict_full_cov / gp_predict_variance call for a shape that is not in
+ *     the schedule cache builds the schedule on the host (0.2 s at n = 32768 / tile 1024, 1.3 s at
+ *     n = 65536 / tile 2048), allocates device memory for it and uploads it with a synchronous
+ *     copy.  Call gp_prepare() first to take that cost up front; after it (or after the first call)
+ *     those entry points only enqueue work and are safe to capture into a CUDA graph.
  *   - Matrices are row-major, 0-based.  n = training points, m = test points
  *     (n-hat in the paper), D = regressors per point, tile = tile edge t with
  *     M = n/tile tiles per dimension.
@@ -197,6 +204,22 @@ int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* s
 int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5);
 /* The same for the schedule of gp_predict_variance (m > 0; no W = V^T V items). */
 int gp_schedule_selfcheck_variance(int64_t n, int64_t m, int tile, int workers, double* stats5);
+
+/* Build and upload, on the current device, the static work-item schedules that gp_cholesky_tiled
+ * (GP_PREPARE_CHOLESKY), gp_predict_full_cov (GP_PREPARE_FULL_COV) and gp_predict_variance
+ * (GP_PREPARE_VARIANCE) need for this shape (step a6: the host-side half of the tile-task scheduler,
+ * PAPER.md:45, 145-147).  Synchronous: blocks the host for the list-scheduling simulation and a
+ * cudaMalloc + cudaMemcpy per schedule.  Idempotent; later compute calls for the same shape find the
+ * schedules in the cache and do not touch the host again.  `what` is an OR of GP_PREPARE_*; m may be 0
+ * for GP_PREPARE_CHOLESKY alone.  *build_ms (host, may be NULL) receives the wall time spent. */
+enum { GP_PREPARE_CHOLESKY = 1, GP_PREPARE_FULL_COV = 2, GP_PREPARE_VARIANCE = 4 };
+int gp_prepare(int64_t n, int64_t m, int tile, int what, double* build_ms);
+
+/* 64-bit fingerprint (FNV-1a over the item list) of the schedule the executor would run for this shape
+ * (m == 0: Cholesky; m > 0: predictor, with or without the Sigma items).  Host only.  Measurements that
+ * depend on the order of work items (the DRAM traffic recorded under profiles/) store it so that
+ * bench.py can tell whether they still describe the current build. */
+int gp_schedule_fingerprint(int64_t n, int64_t m, int tile, int workers, int with_sigma, uint64_t* fingerprint);
 
 /* Drop the cached device-resident schedules (synchronises the device). */
 void gp_release_cached_schedules(void);

@@ -57,7 +57,7 @@ def _load():
         lib.oracle_matvec.argtypes = [dp, i64, i64, dp, dp]
         lib.oracle_forward_subst_cols.argtypes = [dp, i64, dp, i64, dp]
         lib.oracle_posterior_cov.argtypes = [dp, i64, i64, dp, dp]
-        lib.oracle_dense_matvec.argtypes = [dp, i64, dp, dp]
+        lib.oracle_backward_subst_cols.argtypes = [dp, i64, dp, i64, dp]
         lib.oracle_posterior_var.argtypes = [dp, i64, i64, dp, dp]
         lib.oracle_log_marginal_likelihood.argtypes = [dp, i64, dp, dp]
         lib.oracle_log_marginal_likelihood.restype = ctypes.c_double
@@ -157,6 +157,17 @@ def forward_subst_cols(L: np.ndarray, B: np.ndarray) -> np.ndarray:
     V = np.empty_like(B)
     _load().oracle_forward_subst_cols(_p(L), n, _p(B), B.shape[1], _p(V))
     return V
+
+
+def backward_subst_cols(L: np.ndarray, B: np.ndarray) -> np.ndarray:
+    """L^T X = B column by column (PAPER.md:72 recurrence per column); B and X are n x m."""
+    L = _c(L)
+    n = L.shape[0]
+    B = _c(B)
+    assert B.shape[0] == n
+    X = np.empty_like(B)
+    _load().oracle_backward_subst_cols(_p(L), n, _p(B), B.shape[1], _p(X))
+    return X
 
 
 def posterior_cov(V: np.ndarray, Kss: np.ndarray) -> np.ndarray:

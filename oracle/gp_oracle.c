@@ -190,11 +190,29 @@ void oracle_posterior_cov(const double *V, int64_t n, int64_t m, const double *K
     }
 }
 
-/* y = K x for a dense n x n row-major K (used only by the O(n^2) large-n parity probes
- * of DESIGN.md "parity at full size": residual checks that need nothing but a product). */
-void oracle_dense_matvec(const double *K, int64_t n, const double *x, double *y)
+/*
+ * PAPER.md:72 "followed by L^T alpha = beta (backward substitution)" applied to each of the m
+ * columns of the n x m right-hand side B (used by the O(n^2) full-size parity probe of Eq. 3,
+ * Sigma z = K_{X^,X^} z - K_{X^,X} K^-1 K_{X,X^} z with K^-1 applied as two
+ * triangular solves).  Columns are independent, so the OpenMP loop runs over columns; each
+ * column is exactly the recurrence of oracle_backward_subst.  X is n x m.
+ */
+void oracle_backward_subst_cols(const double *L, int64_t n, const double *B, int64_t m, double *X)
 {
-    oracle_matvec(K, n, n, x, y);
+#pragma omp parallel
+    {
+        double *x = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (int64_t c = 0; c < m; ++c) {
+            for (int64_t i = n - 1; i >= 0; --i) {
+                double s = B[i * m + c];
+                for (int64_t p = i + 1; p < n; ++p) s -= L[p * n + i] * x[p];
+                x[i] = s / L[i * n + i];
+            }
+            for (int64_t i = 0; i < n; ++i) X[i * m + c] = x[i];
+        }
+        free(x);
+    }
 }
 
 /*

@@ -23,7 +23,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
-           "gp_schedule_selfcheck_variance")
+           "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint")
 
 
 class gp_hyper(ctypes.Structure):
@@ -83,6 +83,8 @@ def load() -> ctypes.CDLL:
     lib.gp_exec_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ci, vp]
     lib.gp_fp64_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
+    lib.gp_prepare.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.gp_schedule_fingerprint.argtypes = [i64, i64, ci, ci, ci, ctypes.POINTER(ctypes.c_uint64)]
     lib.gp_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
         if name not in ("gp_release_cached_schedules", "gp_strerror"):
@@ -253,6 +255,22 @@ def gp_exec_stats(work: torch.Tensor, max_workers: int = 148):
     if w < 0:
         raise GpError(w, "gp_exec_stats")
     return [tuple(buf[8 * i:8 * i + 8]) for i in range(w)]
+
+
+GP_PREPARE_CHOLESKY, GP_PREPARE_FULL_COV, GP_PREPARE_VARIANCE = 1, 2, 4
+
+
+def gp_prepare(n: int, m: int, tile: int, what: int = GP_PREPARE_CHOLESKY | GP_PREPARE_FULL_COV) -> float:
+    """Build + upload the schedules for this shape on the current device; returns the host time in ms."""
+    ms = ctypes.c_double(0.0)
+    _check(load().gp_prepare(n, m, tile, what, ctypes.byref(ms)), "gp_prepare")
+    return float(ms.value)
+
+
+def gp_schedule_fingerprint(n: int, m: int, tile: int, workers: int = 148, with_sigma: bool = True) -> int:
+    fp = ctypes.c_uint64(0)
+    _check(load().gp_schedule_fingerprint(n, m, tile, workers, int(with_sigma), ctypes.byref(fp)), "gp_schedule_fingerprint")
+    return int(fp.value)
 
 
 def gp_release_cached_schedules() -> None:

@@ -3,6 +3,8 @@
 // No library linear algebra (cuBLAS / cuSOLVER) is linked or called anywhere in this library.
 #include "../../include/gp_b200.h"
 
+#include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -54,14 +56,39 @@ int tile_ok(int64_t n, int tile) {
     return GP_OK;
 }
 
+// Per-device state (the schedule cache is keyed by device, so several devices in one process are
+// supported): SM count and which kernels already had their dynamic shared-memory limit raised.
+constexpr int kMaxDevices = 64;
+std::atomic<int> g_sms[kMaxDevices];
+std::atomic<uint32_t> g_configured[kMaxDevices];
+
+int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) return 0;
+    return dev;
+}
+
 int sm_count() {
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    const int dev = current_device();
+    const int slot = dev < kMaxDevices ? dev : kMaxDevices - 1;
+    int sms = g_sms[slot].load(std::memory_order_relaxed);
+    if (sms == 0 || dev >= kMaxDevices) {
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+        if (dev < kMaxDevices) g_sms[slot].store(sms, std::memory_order_relaxed);
     }
     return sms;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize applies per device: set it once per (device, kernel).
+enum KernelBit : uint32_t { KB_EXEC128 = 1, KB_EXEC64 = 2, KB_EXEC32 = 4, KB_TRTRI128 = 8, KB_TRTRI64 = 16, KB_TRTRI32 = 32,
+                            KB_SOLVE128 = 64, KB_SOLVE64 = 128, KB_SOLVE32 = 256 };
+template <class F>
+int configure_once(uint32_t bit, F&& set) {
+    const int dev = current_device();
+    if (dev < kMaxDevices && (g_configured[dev].load(std::memory_order_acquire) & bit)) return GP_OK;
+    if (!set()) return GP_ERR_CUDA;
+    if (dev < kMaxDevices) g_configured[dev].fetch_or(bit, std::memory_order_release);
+    return GP_OK;
 }
 
 // ---- device-resident schedule cache ---------------------------------------------------------
@@ -70,13 +97,17 @@ struct CachedSchedule {
     int nitems = 0;
 };
 std::mutex g_mu;
-std::map<std::tuple<int, int, int, int, int>, CachedSchedule> g_cache;   // (device, kind, M, Mm, nbt)
+std::map<std::tuple<int, int, int, int, int, int>, CachedSchedule> g_cache;   // (device, kind, M, Mm, nbt, blk)
 
+// kind 0: Cholesky, 1: predictor with Sigma, 2: predictor without (variances only).
+// The first request for a key builds the schedule on the host (list-scheduling simulation: 0.2 s for the
+// n = 32768 / tile 1024 factorisation, 1.3 s for n = 65536 / tile 2048) and uploads it with a synchronous
+// copy; gp_prepare() does this ahead of time so that the compute calls never block (include/gp_b200.h).
 int get_schedule(int kind, int M, int Mm, int nbt, int blk, int workers, CachedSchedule* out) {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
     std::lock_guard<std::mutex> lk(g_mu);
-    auto key = std::make_tuple(dev, kind, M, Mm, nbt);
+    auto key = std::make_tuple(dev, kind, M, Mm, nbt, blk);
     auto it = g_cache.find(key);
     if (it != g_cache.end()) { *out = it->second; return GP_OK; }
     std::vector<SchedItem> items;
@@ -143,12 +174,11 @@ int make_exec_maps(ExecMaps* mp, const ExecParams& p, int b, int64_t m) {
 
 template <int BLK>
 int launch_exec(const ExecParams& p, const ExecMaps& mp, int workers, cudaStream_t st) {
-    static bool configured = false;
     constexpr int smem = exec_smem_bytes<BLK>();
-    if (!configured) {
-        if (cudaFuncSetAttribute(exec_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
-        configured = true;
-    }
+    const int rc = configure_once(BLK == 128 ? KB_EXEC128 : (BLK == 64 ? KB_EXEC64 : KB_EXEC32), [] {
+        return cudaFuncSetAttribute(exec_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+    });
+    if (rc != GP_OK) return rc;
     exec_kernel<BLK><<<workers, kThreads, smem, st>>>(p, mp.L, mp.V, mp.D);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
@@ -166,12 +196,11 @@ int launch_exec_any(int b, const ExecParams& p, int64_t m, int workers, cudaStre
 
 template <int BLK>
 int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStream_t st) {
-    static bool configured = false;
     constexpr int smem = DiagSmem<BLK>::kBytes;
-    if (!configured) {
-        if (cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
-        configured = true;
-    }
+    const int rc = configure_once(BLK == 128 ? KB_TRTRI128 : (BLK == 64 ? KB_TRTRI64 : KB_TRTRI32), [] {
+        return cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+    });
+    if (rc != GP_OK) return rc;
     trtri_diag_kernel<BLK><<<NB, kConsumerThreads, smem, st>>>(L, t, nbt, invD);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
@@ -187,13 +216,12 @@ int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaSt
 template <int SB>
 int launch_solves(const double* dL, int tile, int NB, const double* invD, const double* dY, double* beta, double* dAlpha, int* flags,
                   unsigned int* ticket, cudaStream_t st) {
-    static bool configured = false;
     constexpr int smem = SolveCfg<SB>::kSmemBytes;
-    if (!configured) {
-        if (cudaFuncSetAttribute(forward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
-        if (cudaFuncSetAttribute(backward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return GP_ERR_CUDA;
-        configured = true;
-    }
+    const int rc = configure_once(SB == 128 ? KB_SOLVE128 : (SB == 64 ? KB_SOLVE64 : KB_SOLVE32), [] {
+        return cudaFuncSetAttribute(forward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess &&
+               cudaFuncSetAttribute(backward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
+    });
+    if (rc != GP_OK) return rc;
     forward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
     backward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
@@ -495,6 +523,26 @@ int gp_log_marginal_likelihood(const double* dL, int64_t n, int tile, const doub
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
+int gp_prepare(int64_t n, int64_t m, int tile, int what, double* build_ms) {
+    if (n <= 0 || m < 0 || n > (int64_t)1 << 22 || m > (int64_t)1 << 22) return GP_ERR_SIZE;
+    if ((what & ~(GP_PREPARE_CHOLESKY | GP_PREPARE_FULL_COV | GP_PREPARE_VARIANCE)) != 0 || what == 0) return GP_ERR_MODE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const bool pred = (what & (GP_PREPARE_FULL_COV | GP_PREPARE_VARIANCE)) != 0;
+    if (pred && m <= 0) return GP_ERR_SIZE;
+    if (pred && (rc = tile_ok(m, tile)) != GP_OK) return rc;
+    const int b = pick_block(tile);
+    if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;
+    const int M = (int)(n / tile), Mm = (int)(m / tile), nbt = tile / b;
+    const auto t0 = std::chrono::steady_clock::now();
+    CachedSchedule cs;
+    if ((what & GP_PREPARE_CHOLESKY) && (rc = get_schedule(0, M, 0, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
+    if ((what & GP_PREPARE_FULL_COV) && (rc = get_schedule(1, M, Mm, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
+    if ((what & GP_PREPARE_VARIANCE) && (rc = get_schedule(2, M, Mm, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
+    if (build_ms) *build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return GP_OK;
+}
+
 void gp_release_cached_schedules(void) {
     std::lock_guard<std::mutex> lk(g_mu);
     cudaDeviceSynchronize();
@@ -670,6 +718,21 @@ static int schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, bool 
     }
     const char* why = nullptr;
     return validate_schedule(items, M, Mm, nbt, m > 0, &why, with_sigma) ? GP_OK : GP_ERR_SIZE;
+}
+
+extern "C" int gp_schedule_fingerprint(int64_t n, int64_t m, int tile, int workers, int with_sigma, uint64_t* fingerprint) {
+    if (!fingerprint) return GP_ERR_NULL;
+    if (n <= 0 || m < 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
+    if (workers <= 0) workers = 148;
+    const int b = pick_block(tile), nbt = tile / b, M = (int)(n / tile), Mm = (int)(m / tile);
+    std::vector<SchedItem> items;
+    if (m == 0) build_cholesky_schedule(M, nbt, workers, items, b);
+    else build_predict_schedule(M, Mm, nbt, workers, items, b, nullptr, true, with_sigma != 0);
+    *fingerprint = schedule_fingerprint(items);
+    return GP_OK;
 }
 
 extern "C" int gp_schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, double* stats5) {

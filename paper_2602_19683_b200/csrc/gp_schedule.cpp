@@ -120,10 +120,9 @@ inline SchedItem mk(uint32_t op, int gr, int gc, int q0 = 0, int q1 = 0) {
 // the scheduler keeps the block items of one tile task together so that they share operand panels in L2.
 constexpr int kMergeTail = 2;
 
-int merge_columns() {        // tile columns per trailing-update item
-    static int m = [] { const char* e = std::getenv("GP_B200_MERGE_COLUMNS"); const int v = e ? std::atoi(e) : 4; return v < 1 ? 1 : (v > 4 ? 4 : v); }();
-    return m;
-}
+constexpr int kMergeColumns = 4;     // tile columns per trailing-update item (1..4 measured in round 1: 33.9 / 34.2 / 34.4 / 34.5
+                                     // TFLOP/s at n = 32768; more than 4 gains nothing).  A constant of the build, not a run-time knob.
+constexpr int merge_columns() { return kMergeColumns; }
 
 void program_order_cholesky(int M, int nbt, std::vector<SchedItem>& v, std::vector<int32_t>& task) {
     int32_t tid = 0;
@@ -344,10 +343,38 @@ bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int n
     static const char* kWait = "an item waits for a version no earlier item produces";
     static const char* kFinal = "a block does not end at its final version";
     static const char* kCount = "wrong number of items";
-    bool ok = true;
+    static const char* kInside = "an item waits for a version that a merged update passes without stopping at it";
+    // A merged update raises its block's counter by several versions in steps that are not ordered among the
+    // eight consumer warps (gp_exec.cuh), so the versions strictly inside such a write are never a state in
+    // which the block is complete: nothing may wait for exactly one of them.  `interior` marks them.
+    std::vector<int64_t> multi_blocks;
+    std::vector<int32_t> multi_lo, multi_hi;          // versions lo < v < hi of block multi_blocks[k] are interior
+    {
+        std::vector<int32_t> v2(s.nblocks, 0);
+        for (const SchedItem& it : items) {
+            int64_t blk_written = -1;
+            int count = 0;
+            item_effects(s, it, [](int64_t, int) {}, [&](int64_t b) { if (b == blk_written || blk_written < 0) { blk_written = b; ++count; } });
+            const bool is_upd = it.op == S_UPD_L || it.op == S_UPD_V || it.op == S_UPD_S;
+            if (is_upd && count > 1) { multi_blocks.push_back(blk_written); multi_lo.push_back(v2[blk_written]); multi_hi.push_back(v2[blk_written] + count); }
+            item_effects(s, it, [](int64_t, int) {}, [&](int64_t b) { ++v2[b]; });
+        }
+    }
+    std::vector<int64_t> order(multi_blocks.size());
+    for (size_t k = 0; k < order.size(); ++k) order[k] = (int64_t)k;
+    std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return multi_blocks[a] < multi_blocks[b]; });
+    auto is_interior = [&](int64_t b, int need) {
+        auto lo = std::lower_bound(order.begin(), order.end(), b, [&](int64_t k, int64_t blk) { return multi_blocks[k] < blk; });
+        for (; lo != order.end() && multi_blocks[*lo] == b; ++lo)
+            if (need > multi_lo[*lo] && need < multi_hi[*lo]) return true;
+        return false;
+    };
+    bool ok = true, inside = false;
     for (const SchedItem& it : items) {
-        item_effects(s, it, [&](int64_t b, int need) { if (ver[b] < need) ok = false; }, [&](int64_t b) { ++ver[b]; });
+        item_effects(s, it, [&](int64_t b, int need) { if (ver[b] < need) ok = false; if (need > 0 && is_interior(b, need)) inside = true; },
+                     [&](int64_t b) { ++ver[b]; });
         if (!ok) { if (why) *why = kWait; return false; }
+        if (inside) { if (why) *why = kInside; return false; }
     }
     if (!predict) {
         for (int gr = 0; gr < s.NB; ++gr)
@@ -366,6 +393,14 @@ bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int n
     if (predict) program_order_predict(M, Mm, nbt, with_sigma, prog, task); else program_order_cholesky(M, nbt, prog, task);
     if (prog.size() != items.size()) { if (why) *why = kCount; return false; }
     return true;
+}
+
+uint64_t schedule_fingerprint(const std::vector<SchedItem>& items) {
+    uint64_t h = 1469598103934665603ull;                         // FNV-1a over the item words
+    for (const SchedItem& it : items)
+        for (uint32_t w : {it.op, it.gr, it.gc, it.q})
+            for (int b = 0; b < 4; ++b) { h ^= (w >> (8 * b)) & 0xffu; h *= 1099511628211ull; }
+    return h;
 }
 
 }  // namespace gpb

@@ -7,8 +7,7 @@
 // priority, per-item cost model) decides the order in which items are handed out.  The order is
 // a topological order of the DAG by construction, which is what makes the in-order ticket
 // scheme deadlock-free; the simulated timing only has to be roughly right for waits to be short.
-// Trailing updates of up to four consecutive tile columns are merged into one item per block
-// (environment variable GP_B200_MERGE_COLUMNS = 1..4, default 4, read when the first schedule is built);
+// Trailing updates of four consecutive tile columns are merged into one item per block (a constant of the build);
 // the priority of an item is the critical-path length of its tile task, so that the items in flight
 // share operand panels in L2.
 #pragma once
@@ -43,5 +42,9 @@ void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<Sch
 // earlier in the list) and that every block ends at its final version.  Used by the CPU tests.
 bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why,
                        bool with_sigma = true);
+
+// 64-bit FNV-1a hash of an item list: identifies the schedule a measurement (e.g. an ncu DRAM-traffic
+// capture under profiles/) was taken with.
+uint64_t schedule_fingerprint(const std::vector<SchedItem>& items);
 
 }  // namespace gpb

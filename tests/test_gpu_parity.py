@@ -289,3 +289,37 @@ def test_single_worker_runs_the_whole_dag(gp):
     p = oracle.predict(X, y, Xs, h)
     out = _run_pipeline(gp, X, y, Xs, h, tile, width=1)
     _check_against_oracle(out, p)
+
+
+# ---------------------------------------------------------------- robustness of the inverse-based TRSM
+@pytest.mark.parametrize("noise,cond_floor", [(1e-6, 1e8), (1e-8, 1e10)])
+def test_ill_conditioned_factorisation(gp, noise, cond_floor):
+    """L_IJ = K_IJ inv(L_JJ)^T is a product with an explicit inverse, not a substitution.  On a smooth
+    D=2 problem with tiny noise (cond(K) ~ 6e8 and 6e10, reading A6 allows it) the factor must stay
+    backward stable (||L L^T - K|| / ||K|| at rounding level) and its distance from the oracle must be
+    of the size of the distance between two backward-stable substitution factorisations of the same K
+    (the oracle and LAPACK via numpy): the explicit inverses cost no accuracy that substitution would keep."""
+    n, D, tile = 1024, 2, 256
+    X, y = nfir.nfir_features(77, n, D)
+    h = oracle.Hyper(1.0, 1.0, noise)
+    K = oracle.assemble(X, X, h, True)
+    w = np.linalg.eigvalsh(K)
+    assert w[-1] / w[0] >= cond_floor
+    Lo = oracle.cholesky(K)
+    yardstick = relerr(np.linalg.cholesky(K), Lo)            # ~1e-11 at cond 6e8, ~1e-10 at 6e10
+    pipe = gp.GpPipeline(n, 0, D, tile, gp.Hyper(1.0, 1.0, noise))
+    pipe.assemble(_dev(X))
+    pipe.cholesky()
+    torch.cuda.synchronize()
+    assert int(pipe.info.item()) == 0
+    L = pipe.dense_L().cpu().numpy()
+    resid = np.linalg.norm(L @ L.T - K) / np.linalg.norm(K)
+    err = relerr(L, Lo)
+    print(f"noise={noise:g} cond={w[-1] / w[0]:.3g} residual={resid:.2e} |L-L_oracle|/|L_oracle|={err:.2e} oracle-vs-LAPACK={yardstick:.2e}")
+    assert resid <= 5e-15
+    assert err <= 20 * yardstick
+    # the solve on top of it: K alpha = y to the accuracy cond * u allows
+    pipe.solve(_dev(y))
+    torch.cuda.synchronize()
+    alpha = pipe.alpha.cpu().numpy()
+    assert np.linalg.norm(K @ alpha - y) / (np.linalg.norm(K) * np.linalg.norm(alpha)) <= 1e-14

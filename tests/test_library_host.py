@@ -98,6 +98,38 @@ def test_schedule_headline_config(gp):
     assert st["makespan_us"] <= 1.10 * st["work_us"] / 148
 
 
+def test_schedule_fingerprint_is_stable_and_shape_dependent(gp):
+    a = gp.gp_schedule_fingerprint(1024, 0, 256)
+    assert a == gp.gp_schedule_fingerprint(1024, 0, 256) and a != 0
+    assert a != gp.gp_schedule_fingerprint(1024, 0, 512)
+    assert a != gp.gp_schedule_fingerprint(1024, 1024, 256)
+    assert gp.gp_schedule_fingerprint(1024, 1024, 256, with_sigma=True) != gp.gp_schedule_fingerprint(1024, 1024, 256, with_sigma=False)
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_schedule_fingerprint(1000, 0, 256)
+    assert e.value.code == gp.ERR["TILE"]
+
+
+def test_prepare_validates_arguments_before_touching_the_device(gp):
+    for bad, code in (((1000, 0, 256, 1), "TILE"), ((1024, 1000, 256, 2), "TILE"), ((1024, 0, 256, 2), "SIZE"),
+                      ((1024, 0, 256, 0), "MODE"), ((1024, 0, 256, 8), "MODE"), ((0, 0, 256, 1), "SIZE")):
+        with pytest.raises(gp.GpError) as e:
+            gp.gp_prepare(*bad)
+        assert e.value.code == gp.ERR[code], bad
+
+
+def test_ncu_traffic_record_matches_the_schedule_the_library_builds(gp):
+    """profiles/ncu_traffic.json must describe the CURRENT schedule, otherwise bench.py prints traffic = null."""
+    import json
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        pytest.skip("no ncu traffic record committed yet")
+    for key, rec in json.load(open(path)).items():
+        n, tile = (int(x.split("=")[1]) for x in key.split(","))
+        assert rec["schedule_fingerprint"] == "%016x" % gp.gp_schedule_fingerprint(n, 0, tile, 148), key
+        assert rec["dram_bytes"] > 0 and rec["source"].startswith("profiles/")
+        assert os.path.exists(os.path.join(ROOT, rec["source"].split(" ")[0]))
+
+
 def test_binding_refuses_cpu_tensors(gp):
     import torch
     X = torch.zeros(32, 2, dtype=torch.float64)

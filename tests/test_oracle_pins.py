@@ -134,6 +134,14 @@ def test_cholesky_and_substitutions_vs_numpy_scipy(n):
     np.testing.assert_allclose(oracle.backward_subst(L, b), scipy.linalg.solve_triangular(L.T, b, lower=False), rtol=1e-11)
     B = rng.normal(size=(n, 7))
     np.testing.assert_allclose(oracle.forward_subst_cols(L, B), scipy.linalg.solve_triangular(L, B, lower=True), rtol=1e-11)
+    # the multi-column backward substitution: against the library routine (a transposed-operand or wrong-direction
+    # slip fails here), and bit-identical to the single-vector recurrence column by column
+    Xb = oracle.backward_subst_cols(L, B)
+    np.testing.assert_allclose(Xb, scipy.linalg.solve_triangular(L.T, B, lower=False), rtol=1e-11)
+    for c in range(B.shape[1]):
+        assert np.array_equal(Xb[:, c], oracle.backward_subst(L, np.ascontiguousarray(B[:, c])))
+    # forward then backward = K^-1: K (L^-T L^-1 B) = B
+    np.testing.assert_allclose(K @ oracle.backward_subst_cols(L, oracle.forward_subst_cols(L, B)), B, rtol=1e-9, atol=1e-11)
     M = rng.normal(size=(9, n))
     np.testing.assert_allclose(oracle.matvec(M, b), M @ b, rtol=1e-12, atol=1e-13)
     V = rng.normal(size=(n, 6))

@@ -56,3 +56,15 @@ def test_reference_arm_under_torchrun_prints_one_line():
     d = lines[0]
     assert d["impl"] == "reference" and d["value"] > 0 and d["unit"] == "GFLOP/s"
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["e2e"]["unit"] == "GFLOP/s" == sys.modules.get("bench", __import__("bench")).E2E_UNIT
+    # config 1 is small enough for the oracle to run the config itself: the workload string is not a sample
+    assert d["config"]["workload"].startswith("c1:") and "sample_n" not in d["config"]
+
+
+def test_reference_arm_names_the_sample_it_runs():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2602_19683_b200 import nfir
+    n, m, sampled = bench.reference_sample(nfir.CONFIGS[3])
+    assert sampled and (n, m) == bench.ORACLE_SAMPLE
+    assert bench.reference_sample(nfir.CONFIGS[0]) == (128, 128, False)

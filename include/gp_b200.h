@@ -221,6 +221,17 @@ int gp_prepare(int64_t n, int64_t m, int tile, int what, double* build_ms);
  * bench.py can tell whether they still describe the current build. */
 int gp_schedule_fingerprint(int64_t n, int64_t m, int tile, int workers, int with_sigma, uint64_t* fingerprint);
 
+/* Scheduling granularity (step a6; the analogue of the paper's "tiles per dimension" knob).
+ * The tile tasks of Fig. 1 are formed over scheduling tiles of g x g blocks (block = gp_block_size(tile)); g is
+ * independent of the storage tile.  gp_schedule_granularity() returns the g the library uses for a shape:
+ * auto = 1 up to 96 block columns (short serial chains while the critical path bounds the run), else about 32
+ * scheduling tiles per dimension (long work items whose panels are shared in L2).  Results do not depend on g
+ * beyond rounding order.  gp_set_schedule_granularity(blocks) overrides the choice for later calls of this
+ * process (0 = auto again; the largest divisor of the block counts <= blocks is used): measurement support
+ * for bench.py --sweep, not needed in normal use. */
+int gp_set_schedule_granularity(int blocks);
+int gp_schedule_granularity(int64_t n, int64_t m, int tile);
+
 /* Drop the cached device-resident schedules (synchronises the device). */
 void gp_release_cached_schedules(void);
 

@@ -23,7 +23,8 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
-           "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint")
+           "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
+           "gp_set_schedule_granularity", "gp_schedule_granularity")
 
 
 class gp_hyper(ctypes.Structure):
@@ -85,6 +86,8 @@ def load() -> ctypes.CDLL:
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
     lib.gp_prepare.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_schedule_fingerprint.argtypes = [i64, i64, ci, ci, ci, ctypes.POINTER(ctypes.c_uint64)]
+    lib.gp_set_schedule_granularity.argtypes = [ci]
+    lib.gp_schedule_granularity.argtypes = [i64, i64, ci]
     lib.gp_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
         if name not in ("gp_release_cached_schedules", "gp_strerror"):
@@ -271,6 +274,18 @@ def gp_schedule_fingerprint(n: int, m: int, tile: int, workers: int = 148, with_
     fp = ctypes.c_uint64(0)
     _check(load().gp_schedule_fingerprint(n, m, tile, workers, int(with_sigma), ctypes.byref(fp)), "gp_schedule_fingerprint")
     return int(fp.value)
+
+
+def gp_set_schedule_granularity(blocks: int) -> None:
+    """Override the scheduling-tile edge in blocks for later calls (0 = auto); measurement support."""
+    _check(load().gp_set_schedule_granularity(int(blocks)), "gp_set_schedule_granularity")
+
+
+def gp_schedule_granularity(n: int, m: int, tile: int) -> int:
+    g = int(load().gp_schedule_granularity(n, m, tile))
+    if g < 0:
+        raise GpError(g, "gp_schedule_granularity")
+    return g
 
 
 def gp_release_cached_schedules() -> None:

@@ -50,6 +50,28 @@ HyperDev to_dev(const gp_hyper& h) {
     return d;
 }
 
+// ---- scheduling granularity ---------------------------------------------------------------------
+// The tile tasks of PAPER.md Fig. 1 are formed over SCHEDULING tiles of g x g blocks; g is the library's
+// choice and independent of the storage tile of the API.  Small g = short serial chains (the TRSM tile task
+// of a block row is a chain of g dependent block solves): best while the critical path bounds the run
+// (measured at n = 8192: g = 1 / 2 / 4 / 8 -> 7.45 / 8.15 / 8.61 / 10.2 ms).  Large g = fewer, longer work
+// items whose operand panels are shared in L2: best once the trailing updates dominate (n = 32768, g = 8:
+// 93 % of the FP64 peak).  Auto: g = 1 up to 96 block columns, else the largest divisor of the block counts
+// that keeps about 32 scheduling tiles per dimension.
+std::atomic<int> g_sched_blocks{0};      // 0 = auto; set by gp_set_schedule_granularity (measurement support)
+
+int gcd_int(int a, int b) { while (b) { const int t = a % b; a = b; b = t; } return a; }
+
+int pick_sched_blocks(int NB, int NBm) {
+    const int common = NBm > 0 ? gcd_int(NB, NBm) : NB;
+    int want = g_sched_blocks.load(std::memory_order_relaxed);
+    if (want <= 0) want = NB <= 96 ? 1 : NB / 32;
+    int g = 1;
+    for (int d = 1; d <= want && d <= common; ++d)
+        if (common % d == 0) g = d;
+    return g;
+}
+
 int tile_ok(int64_t n, int tile) {
     if (tile <= 0 || tile % 32 != 0) return GP_ERR_TILE;
     if (n % tile != 0) return GP_ERR_TILE;
@@ -351,7 +373,8 @@ int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* w
     if (tile_tasks) *tile_tasks = M + M * (M - 1) / 2 + M * (M - 1) / 2 + M * (M - 1) * (M - 2) / 6;
     if (work_items) {
         std::vector<SchedItem> items;
-        build_cholesky_schedule((int)M, tile / pick_block(tile), 148, items, pick_block(tile), nullptr, false);
+        const int b = pick_block(tile), NB = (int)(n / b), g = pick_sched_blocks(NB, 0);
+        build_cholesky_schedule(NB / g, g, 148, items, b, nullptr, false);
         *work_items = (int64_t)items.size();
     }
     return GP_OK;
@@ -369,8 +392,9 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     cudaStream_t st = (cudaStream_t)stream;
     const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b);
     const int workers = workers_for(sched_width);
+    const int g = pick_sched_blocks(NB, 0);
     CachedSchedule cs;
-    rc = get_schedule(0, M, 0, nbt, b, sm_count(), &cs);
+    rc = get_schedule(0, NB / g, 0, g, b, sm_count(), &cs);
     if (rc != GP_OK) return rc;
     char* ws = (char*)dWork;
     if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;        // ticket + version counters
@@ -387,6 +411,7 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     p.d_info = d_info;
     p.t = tile;
     p.nbt = nbt;
+    p.snbt = g;
     p.NB = NB;
     p.Mt = M;
     return launch_exec_any(b, p, 0, workers, st);
@@ -446,10 +471,11 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     const CovWs w = cov_ws(n, m, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    const int M = (int)(n / tile), Mm = (int)(m / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
+    const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
     const int workers = workers_for(sched_width);
+    const int g = pick_sched_blocks(NB, NBm);
     CachedSchedule cs;
-    rc = get_schedule(dSigma ? 1 : 2, M, Mm, nbt, b, sm_count(), &cs);
+    rc = get_schedule(dSigma ? 1 : 2, NB / g, NBm / g, g, b, sm_count(), &cs);
     if (rc != GP_OK) return rc;
     char* ws = (char*)dWork;
     const HyperDev hd = to_dev(h);
@@ -484,6 +510,7 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     p.stats = (unsigned long long*)(ws + kStatsOff);
     p.t = tile;
     p.nbt = nbt;
+    p.snbt = g;
     p.NB = NB;
     p.NBm = NBm;
     p.Mt = M;
@@ -533,14 +560,30 @@ int gp_prepare(int64_t n, int64_t m, int tile, int what, double* build_ms) {
     if (pred && (rc = tile_ok(m, tile)) != GP_OK) return rc;
     const int b = pick_block(tile);
     if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;
-    const int M = (int)(n / tile), Mm = (int)(m / tile), nbt = tile / b;
+    const int NB = (int)(n / b), NBm = (int)(m / b);
+    const int gc = pick_sched_blocks(NB, 0), gp = pred ? pick_sched_blocks(NB, NBm) : 1;
     const auto t0 = std::chrono::steady_clock::now();
     CachedSchedule cs;
-    if ((what & GP_PREPARE_CHOLESKY) && (rc = get_schedule(0, M, 0, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
-    if ((what & GP_PREPARE_FULL_COV) && (rc = get_schedule(1, M, Mm, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
-    if ((what & GP_PREPARE_VARIANCE) && (rc = get_schedule(2, M, Mm, nbt, b, sm_count(), &cs)) != GP_OK) return rc;
+    if ((what & GP_PREPARE_CHOLESKY) && (rc = get_schedule(0, NB / gc, 0, gc, b, sm_count(), &cs)) != GP_OK) return rc;
+    if ((what & GP_PREPARE_FULL_COV) && (rc = get_schedule(1, NB / gp, NBm / gp, gp, b, sm_count(), &cs)) != GP_OK) return rc;
+    if ((what & GP_PREPARE_VARIANCE) && (rc = get_schedule(2, NB / gp, NBm / gp, gp, b, sm_count(), &cs)) != GP_OK) return rc;
     if (build_ms) *build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     return GP_OK;
+}
+
+int gp_set_schedule_granularity(int blocks) {
+    if (blocks < 0 || blocks > 4096) return GP_ERR_SIZE;
+    g_sched_blocks.store(blocks, std::memory_order_relaxed);
+    return GP_OK;
+}
+
+int gp_schedule_granularity(int64_t n, int64_t m, int tile) {
+    if (n <= 0 || m < 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
+    const int b = pick_block(tile);
+    return pick_sched_blocks((int)(n / b), (int)(m / b));
 }
 
 void gp_release_cached_schedules(void) {
@@ -680,6 +723,7 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
     p.d_info = (int*)(ws + align_up(tiles_bytes, 256) + 128);
     p.t = K;
     p.nbt = nbt;
+    p.snbt = nbt;
     p.NB = NB;
     p.Mt = M;
     p.no_deps = 1;
@@ -704,7 +748,8 @@ static int schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, bool 
     if (rc != GP_OK) return rc;
     if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
     if (workers <= 0) workers = 148;
-    const int b = pick_block(tile), nbt = tile / b, M = (int)(n / tile), Mm = (int)(m / tile);
+    const int b = pick_block(tile), NB = (int)(n / b), NBm = (int)(m / b), nbt = pick_sched_blocks(NB, NBm);
+    const int M = NB / nbt, Mm = NBm / nbt;
     std::vector<SchedItem> items;
     SchedStats st;
     if (m == 0) build_cholesky_schedule(M, nbt, workers, items, b, &st, true);
@@ -727,10 +772,10 @@ extern "C" int gp_schedule_fingerprint(int64_t n, int64_t m, int tile, int worke
     if (rc != GP_OK) return rc;
     if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
     if (workers <= 0) workers = 148;
-    const int b = pick_block(tile), nbt = tile / b, M = (int)(n / tile), Mm = (int)(m / tile);
+    const int b = pick_block(tile), NB = (int)(n / b), NBm = (int)(m / b), g = pick_sched_blocks(NB, NBm);
     std::vector<SchedItem> items;
-    if (m == 0) build_cholesky_schedule(M, nbt, workers, items, b);
-    else build_predict_schedule(M, Mm, nbt, workers, items, b, nullptr, true, with_sigma != 0);
+    if (m == 0) build_cholesky_schedule(NB / g, g, workers, items, b);
+    else build_predict_schedule(NB / g, NBm / g, g, workers, items, b, nullptr, true, with_sigma != 0);
     *fingerprint = schedule_fingerprint(items);
     return GP_OK;
 }

@@ -65,7 +65,10 @@ struct ExecParams {
     int* d_info;
     int nitems;
     int t;                 // tile edge
-    int nbt;               // blocks per tile edge (t / b)
+    int nbt;               // blocks per tile edge (t / b): ADDRESSING only (the storage tile of the API)
+    int snbt;              // blocks per SCHEDULING tile: the tile tasks of Fig. 1 are formed over virtual tiles of snbt x snbt
+                           // blocks, chosen by the library for the problem size and independent of the storage tile
+                           // (gp_api.cu, pick_sched_blocks); version counting, ROW chains and column merging use this one
     int NB;                // n / b
     int NBm;               // m / b
     int Mt;                // n / t (tiles per row of V^T)
@@ -149,10 +152,10 @@ struct Producer {
     }
     // number of writes after which block (gr,gc) of L is final
     __device__ __forceinline__ int finL(int gr, int gc) const {
-        const int K = gc / p.nbt, bk = gc % p.nbt;
-        return (gr / p.nbt == K) ? K + 1 + bk : K + 1 + (bk > 0 ? 1 : 0);
+        const int K = gc / p.snbt, bk = gc % p.snbt;
+        return (gr / p.snbt == K) ? K + 1 + bk : K + 1 + (bk > 0 ? 1 : 0);
     }
-    __device__ __forceinline__ int finV(int gc) const { return gc / p.nbt + 1 + (gc % p.nbt > 0 ? 1 : 0); }
+    __device__ __forceinline__ int finV(int gc) const { return gc / p.snbt + 1 + (gc % p.snbt > 0 ? 1 : 0); }
 
     // ---- dependency polling: wait w of the current job is handled by lane w % 32 ------------------
     __device__ __forceinline__ void poll(const int* addr, int need) {
@@ -185,12 +188,13 @@ struct Producer {
         if (++slot == kJobSlots) { slot = 0; jphase ^= 1; }
     }
     // `C`/`ldc` (may be null): the block the consumers will read in their epilogue.  Its rows are pulled into
-    // L2 with cp.async.bulk.prefetch.L2 a few stages before the end of the job -- early enough to hide the
-    // HBM latency, late enough not to be evicted again (at job start, ~140 us earlier, it was).
+    // L2 with cp.async.bulk.prefetch.L2 at the start of this call; the caller passes it with the block that is
+    // streamed two blocks (16 stages) before the end of the job -- early enough to hide the HBM latency, late
+    // enough not to be evicted again (at job start, ~140 us earlier, it was).
     __device__ __forceinline__ void stream(const CUtensorMap* mA, int2 a, const CUtensorMap* mB, int2 b, int nk,
                                            const double* C = nullptr, int ldc = 0) {
         if (lane != 0) return;
-        const int kpre = nk > kPrefetchLead ? nk - kPrefetchLead : 0;
+        const int kpre = 0;                    // the caller picks the block at which the prefetch is due
         for (int kt = 0; kt < nk; ++kt) {
             mbar_wait(&empty[stage], (uint32_t)(phase ^ 1), 2);
             char* dst = ring + (size_t)stage * Cfg::kStageBytes;
@@ -215,15 +219,15 @@ struct Producer {
                 const int* addr = nullptr;
                 int need = 0;
                 if (op == OP_UPD_L) {
-                    if (w == 0) { addr = p.verL + (size_t)gr * p.NB + gc; need = q0 / p.nbt + q0 % p.nbt; }
+                    if (w == 0) { addr = p.verL + (size_t)gr * p.NB + gc; need = q0 / p.snbt + q0 % p.snbt; }
                     else if (w <= nq) { const int q = q0 + w - 1; addr = p.verL + (size_t)gr * p.NB + q; need = finL(gr, q); }
                     else { const int q = q0 + w - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
                 } else if (op == OP_UPD_V) {
-                    if (w == 0) { addr = p.verV + (size_t)gr * p.NB + gc; need = q0 / p.nbt; }
+                    if (w == 0) { addr = p.verV + (size_t)gr * p.NB + gc; need = q0 / p.snbt; }
                     else if (w <= nq) { const int q = q0 + w - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
                     else if (!p.L_final) { const int q = q0 + w - 1 - nq; addr = p.verL + (size_t)gc * p.NB + q; need = finL(gc, q); }
                 } else {  // OP_UPD_S
-                    if (w == 0) { addr = p.verS + (size_t)gr * p.NBm + gc; need = q0 / p.nbt; }
+                    if (w == 0) { addr = p.verS + (size_t)gr * p.NBm + gc; need = q0 / p.snbt; }
                     else if (w <= nq) { const int q = q0 + w - 1; addr = p.verV + (size_t)gr * p.NB + q; need = finV(q); }
                     else { const int q = q0 + w - 1 - nq; addr = p.verV + (size_t)gc * p.NB + q; need = finV(q); }
                 }
@@ -232,31 +236,23 @@ struct Producer {
         }
         deps_done(t0);
         const int nk = nq * BLK / kBK;
+        // merged tile columns: one job, one version per column.  The panels are streamed block by block (a block
+        // is contiguous in the TMA view of its storage tile; a run of blocks need not be: the scheduling tile is
+        // independent of the storage tile), and the C block is prefetched into L2 two blocks before the end.
+        const int ncol = nq > p.snbt ? nq / p.snbt : 1;
+        const int qpre = nq > 2 ? q1 - 2 : q0;
         if (op == OP_UPD_L) {
             double* C = blkL(gr, gc);
-            // merged tile columns: one job, one version per column, the panels streamed column by column
-            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
             push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
-            for (int c = 0; c < ncol; ++c) {
-                const int q = q0 + c * p.nbt;
-                stream(mapL, crdL(gr, q), mapL, crdL(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, p.t);
-            }
+            for (int q = q0; q < q1; ++q) stream(mapL, crdL(gr, q), mapL, crdL(gc, q), BLK / kBK, q == qpre ? C : nullptr, p.t);
         } else if (op == OP_UPD_V) {
             double* C = blkV(gr, gc);
-            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
             push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
-            for (int c = 0; c < ncol; ++c) {
-                const int q = q0 + c * p.nbt;
-                stream(mapV, crdV(gr, q), mapL, crdL(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, p.t);
-            }
+            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapL, crdL(gc, q), BLK / kBK, q == qpre ? C : nullptr, p.t);
         } else {
             double* C = blkS(gr, gc);
-            const int ncol = nq > p.nbt ? nq / p.nbt : 1;
             push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, ncol);
-            for (int c = 0; c < ncol; ++c) {
-                const int q = q0 + c * p.nbt;
-                stream(mapV, crdV(gr, q), mapV, crdV(gc, q), nk / ncol, c + 1 == ncol ? C : nullptr, (int)p.m);
-            }
+            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapV, crdV(gc, q), BLK / kBK, q == qpre ? C : nullptr, (int)p.m);
         }
     }
 
@@ -283,7 +279,7 @@ struct Producer {
     }
 
     __device__ void row_chain(bool is_v, int gr, int qt) {
-        for (int jj = 0; jj < p.nbt; ++jj) {
+        for (int jj = 0; jj < p.snbt; ++jj) {
             if (jj > 0) update(is_v ? OP_UPD_V : OP_UPD_L, gr, qt + jj, qt, qt + jj);
             trsm(is_v, gr, qt + jj);
         }

@@ -40,7 +40,6 @@ constexpr int kProducerRegs = 56;
 constexpr int kBK = 16;                           // contraction depth per stage = one 128-byte swizzle row
 constexpr int kStages = 7;                       // 7 x 32 KB (b = 128) + barriers fits the 227 KB of an SM; one stage is always held back (deferred release)
 constexpr int kJobSlots = 4;
-constexpr int kPrefetchLead = 12;                 // k-stages before the end of a job at which its C block is prefetched into L2
 
 template <int BLK>
 struct GemmCfg {

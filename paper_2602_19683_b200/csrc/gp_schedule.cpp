@@ -90,9 +90,9 @@ void item_effects(const Shape& s, const SchedItem& it, FW&& wait, FR&& write) {
 struct Cost {
     double per_q, fixed, potrf;
     explicit Cost(int blk) {
-        if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 80.0; }
-        else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 14.0; }
-        else { per_q = 0.8; fixed = 2.5; potrf = 6.0; }
+        if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 40.0; }     // potrf: the r02 diagonal block (38 us measured)
+        else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 16.0; }
+        else { per_q = 0.8; fixed = 2.5; potrf = 7.0; }
     }
     double of(const SchedItem& it, int nbt) const {
         const int q0 = (int)(it.q & 0xffffu), q1 = (int)(it.q >> 16);

@@ -101,12 +101,35 @@ def test_schedule_headline_config(gp):
 def test_schedule_fingerprint_is_stable_and_shape_dependent(gp):
     a = gp.gp_schedule_fingerprint(1024, 0, 256)
     assert a == gp.gp_schedule_fingerprint(1024, 0, 256) and a != 0
-    assert a != gp.gp_schedule_fingerprint(1024, 0, 512)
+    assert a == gp.gp_schedule_fingerprint(1024, 0, 512)      # same blocks, same scheduling tile: the storage tile does not matter
+    assert a != gp.gp_schedule_fingerprint(2048, 0, 256)
     assert a != gp.gp_schedule_fingerprint(1024, 1024, 256)
     assert gp.gp_schedule_fingerprint(1024, 1024, 256, with_sigma=True) != gp.gp_schedule_fingerprint(1024, 1024, 256, with_sigma=False)
     with pytest.raises(gp.GpError) as e:
         gp.gp_schedule_fingerprint(1000, 0, 256)
     assert e.value.code == gp.ERR["TILE"]
+
+
+def test_schedule_granularity_auto_and_override(gp):
+    # auto: 1 scheduling block up to 96 block columns, then about 32 scheduling tiles per dimension
+    assert gp.gp_schedule_granularity(1024, 1024, 256) == 1
+    assert gp.gp_schedule_granularity(8192, 1024, 512) == 1
+    assert gp.gp_schedule_granularity(32768, 4096, 1024) == 8
+    assert gp.gp_schedule_granularity(65536, 8192, 2048) == 16
+    assert gp.gp_schedule_granularity(32768, 0, 128) == 8        # independent of the storage tile
+    try:
+        for g in (1, 2, 4, 8):
+            gp.gp_set_schedule_granularity(g)
+            assert gp.gp_schedule_granularity(8192, 1024, 512) == g
+            for (n, m) in ((8192, 0), (8192, 1024)):
+                rc, st = gp.gp_schedule_selfcheck(n, m, 512, 148)
+                assert rc == 0 and st["items"] > 0
+        gp.gp_set_schedule_granularity(3)                          # not a divisor of 64: the largest divisor below it
+        assert gp.gp_schedule_granularity(8192, 1024, 512) == 2
+    finally:
+        gp.gp_set_schedule_granularity(0)
+    with pytest.raises(gp.GpError):
+        gp.gp_set_schedule_granularity(-1)
 
 
 def test_prepare_validates_arguments_before_touching_the_device(gp):

@@ -235,8 +235,17 @@ int gp_schedule_granularity(int64_t n, int64_t m, int tile);
 /* Drop the cached device-resident schedules (synchronises the device). */
 void gp_release_cached_schedules(void);
 
-/* Size in doubles of the CTA-level block the tile tasks are split into for this tile size. */
+/* Edge (in doubles) of the largest CTA-level block this tile size admits: 128 if tile % 128 == 0, else 64 if
+ * tile % 64 == 0, else 32. */
 int gp_block_size(int tile);
+/* Edge of the block the library actually splits the tile tasks into for an n x n problem with this tile size:
+ * the largest admissible edge up to 64 for n <= 8192 (short serial chains while the critical path bounds the run),
+ * up to 128 beyond (full contraction rate).  The storage tile only fixes the addressing; results do not depend on
+ * the block edge beyond rounding order.  gp_set_block_edge(b) (b in {0 = auto, 32, 64, 128}) overrides the cap for
+ * later calls of this process -- call it before gp_workspace_bytes, whose sizes depend on the block edge;
+ * measurement support for bench.py --sweep. */
+int gp_block_size_for(int64_t n, int tile);
+int gp_set_block_edge(int b);
 
 const char* gp_strerror(int code);
 

@@ -24,7 +24,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
-           "gp_set_schedule_granularity", "gp_schedule_granularity")
+           "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge")
 
 
 class gp_hyper(ctypes.Structure):
@@ -86,6 +86,8 @@ def load() -> ctypes.CDLL:
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
     lib.gp_prepare.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_schedule_fingerprint.argtypes = [i64, i64, ci, ci, ci, ctypes.POINTER(ctypes.c_uint64)]
+    lib.gp_block_size_for.argtypes = [i64, ci]
+    lib.gp_set_block_edge.argtypes = [ci]
     lib.gp_set_schedule_granularity.argtypes = [ci]
     lib.gp_schedule_granularity.argtypes = [i64, i64, ci]
     lib.gp_strerror.restype = ctypes.c_char_p
@@ -274,6 +276,15 @@ def gp_schedule_fingerprint(n: int, m: int, tile: int, workers: int = 148, with_
     fp = ctypes.c_uint64(0)
     _check(load().gp_schedule_fingerprint(n, m, tile, workers, int(with_sigma), ctypes.byref(fp)), "gp_schedule_fingerprint")
     return int(fp.value)
+
+
+def gp_block_size_for(n: int, tile: int) -> int:
+    return int(load().gp_block_size_for(int(n), int(tile)))
+
+
+def gp_set_block_edge(b: int) -> None:
+    """Override the cap on the block edge (0 = auto, 32, 64, 128); call before allocating workspaces."""
+    _check(load().gp_set_block_edge(int(b)), "gp_set_block_edge")
 
 
 def gp_set_schedule_granularity(blocks: int) -> None:

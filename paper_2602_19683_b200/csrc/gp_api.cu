@@ -30,9 +30,19 @@ constexpr size_t kHdrBytes = 16384;
 constexpr size_t kStatsBytes = 64;   // 8 uint64 per worker, see gp_exec_stats
 constexpr int kMaxWorkers = (int)((kHdrBytes - kStatsOff) / kStatsBytes);
 
-int pick_block(int tile) {
-    if (tile % 128 == 0) return 128;
-    if (tile % 64 == 0) return 64;
+// Block edge b: the unit of work and of dependency tracking inside a storage tile (any b in {128, 64, 32} that
+// divides the tile works; the tile only fixes the addressing).  128-blocks give the contraction its full rate
+// (93 % of the FP64 peak at n = 32768) but every step of the serial spine -- POTRF of a diagonal block, TRSM of
+// the block below, update of the next diagonal block -- is then 38 + 24 + 24 us; with 64-blocks it is
+// 15 + 7 + 7 us per 64 columns.  Measured Cholesky, b = 64 vs 128: n = 1024: 0.47 / 0.70 ms, 4096: 1.88 / 2.94,
+// 6144: 3.96 / 4.58, 8192: 7.17 / 7.43, 16384: the 128-block wins.  So: 64 up to n = 8192, else 128.
+std::atomic<int> g_block_edge{0};        // 0 = auto; set by gp_set_block_edge (measurement support)
+
+int pick_block(int tile, int64_t n) {
+    int cap = g_block_edge.load(std::memory_order_relaxed);
+    if (cap <= 0) cap = n <= 8192 ? 64 : 128;
+    if (cap >= 128 && tile % 128 == 0) return 128;
+    if (cap >= 64 && tile % 64 == 0) return 64;
     return 32;
 }
 
@@ -309,7 +319,20 @@ extern "C" {
 
 int gp_block_size(int tile) {
     if (tile <= 0 || tile % 32 != 0) return GP_ERR_TILE;
-    return pick_block(tile);
+    return tile % 128 == 0 ? 128 : (tile % 64 == 0 ? 64 : 32);
+}
+
+int gp_block_size_for(int64_t n, int tile) {
+    if (n <= 0) return GP_ERR_SIZE;
+    const int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    return pick_block(tile, n);
+}
+
+int gp_set_block_edge(int b) {
+    if (b != 0 && b != 32 && b != 64 && b != 128) return GP_ERR_SIZE;
+    g_block_edge.store(b, std::memory_order_relaxed);
+    return GP_OK;
 }
 
 const char* gp_strerror(int code) {
@@ -331,7 +354,7 @@ int gp_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* chol, size
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
     if (m > 0 && m % tile != 0) return GP_ERR_TILE;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     if (chol) *chol = chol_ws(n, b).total;
     if (solve) *solve = solve_ws(n, b).total;
     if (full_cov) *full_cov = m > 0 ? cov_ws(n, m, b).total : 0;
@@ -373,7 +396,7 @@ int gp_cholesky_task_counts(int64_t n, int tile, int64_t* tile_tasks, int64_t* w
     if (tile_tasks) *tile_tasks = M + M * (M - 1) / 2 + M * (M - 1) / 2 + M * (M - 1) * (M - 2) / 6;
     if (work_items) {
         std::vector<SchedItem> items;
-        const int b = pick_block(tile), NB = (int)(n / b), g = pick_sched_blocks(NB, 0);
+        const int b = pick_block(tile, n), NB = (int)(n / b), g = pick_sched_blocks(NB, 0);
         build_cholesky_schedule(NB / g, g, 148, items, b, nullptr, false);
         *work_items = (int64_t)items.size();
     }
@@ -385,7 +408,7 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
     if (n <= 0 || n > (int64_t)1 << 22) return GP_ERR_SIZE;
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     if (n / b > 65535) return GP_ERR_SIZE;            // block indices travel in 16 bits of a work item
     const CholWs w = chol_ws(n, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
@@ -423,7 +446,7 @@ int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dA
     if (n <= 0) return GP_ERR_SIZE;
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     const SolveWs w = solve_ws(n, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -466,7 +489,7 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     rc = tile_ok(m, tile);
     if (rc != GP_OK) return rc;
     if (!hyper_ok(h)) return GP_ERR_HYPER;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;   // block indices travel in 16 bits of a work item
     const CovWs w = cov_ws(n, m, b);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
@@ -558,7 +581,7 @@ int gp_prepare(int64_t n, int64_t m, int tile, int what, double* build_ms) {
     const bool pred = (what & (GP_PREPARE_FULL_COV | GP_PREPARE_VARIANCE)) != 0;
     if (pred && m <= 0) return GP_ERR_SIZE;
     if (pred && (rc = tile_ok(m, tile)) != GP_OK) return rc;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;
     const int NB = (int)(n / b), NBm = (int)(m / b);
     const int gc = pick_sched_blocks(NB, 0), gp = pred ? pick_sched_blocks(NB, NBm) : 1;
@@ -582,7 +605,7 @@ int gp_schedule_granularity(int64_t n, int64_t m, int tile) {
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
     if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
-    const int b = pick_block(tile);
+    const int b = pick_block(tile, n);
     return pick_sched_blocks((int)(n / b), (int)(m / b));
 }
 
@@ -748,7 +771,7 @@ static int schedule_selfcheck(int64_t n, int64_t m, int tile, int workers, bool 
     if (rc != GP_OK) return rc;
     if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
     if (workers <= 0) workers = 148;
-    const int b = pick_block(tile), NB = (int)(n / b), NBm = (int)(m / b), nbt = pick_sched_blocks(NB, NBm);
+    const int b = pick_block(tile, n), NB = (int)(n / b), NBm = (int)(m / b), nbt = pick_sched_blocks(NB, NBm);
     const int M = NB / nbt, Mm = NBm / nbt;
     std::vector<SchedItem> items;
     SchedStats st;
@@ -772,7 +795,7 @@ extern "C" int gp_schedule_fingerprint(int64_t n, int64_t m, int tile, int worke
     if (rc != GP_OK) return rc;
     if (m > 0 && (rc = tile_ok(m, tile)) != GP_OK) return rc;
     if (workers <= 0) workers = 148;
-    const int b = pick_block(tile), NB = (int)(n / b), NBm = (int)(m / b), g = pick_sched_blocks(NB, NBm);
+    const int b = pick_block(tile, n), NB = (int)(n / b), NBm = (int)(m / b), g = pick_sched_blocks(NB, NBm);
     std::vector<SchedItem> items;
     if (m == 0) build_cholesky_schedule(NB / g, g, workers, items, b);
     else build_predict_schedule(NB / g, NBm / g, g, workers, items, b, nullptr, true, with_sigma != 0);

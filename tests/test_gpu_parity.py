@@ -28,6 +28,16 @@ def _dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
+@pytest.fixture(autouse=True)
+def _auto_tuning(gp):
+    """Every test starts and ends with the library's own choice of block edge and scheduling granularity."""
+    gp.gp_set_block_edge(0)
+    gp.gp_set_schedule_granularity(0)
+    yield
+    gp.gp_set_block_edge(0)
+    gp.gp_set_schedule_granularity(0)
+
+
 def _run_pipeline(gp, X, y, Xs, h, tile, width=0):
     n, D = X.shape
     m = Xs.shape[0]
@@ -77,10 +87,30 @@ def test_configs_full_pipeline(gp, ci):
     (320, 320, 8, 160),     # tile 160 -> block 32, 5 blocks per tile edge
 ])
 def test_shapes_spanning_tiles_and_blocks(gp, n, m, D, tile):
+    """Each shape with the library's own block edge (64 or 32 at these sizes) and with the 128-block path the
+    large configurations use forced on (where the tile admits it)."""
     X, y = nfir.nfir_features(n + m + D, n, D)
     Xs, _ = nfir.nfir_features(7 * n + 1, m, D, with_targets=False)
     h = oracle.Hyper()
     p = oracle.predict(X, y, Xs, h)
+    for cap in (0, 128):
+        gp.gp_set_block_edge(cap)
+        out = _run_pipeline(gp, X, y, Xs, h, tile)
+        _check_against_oracle(out, p)
+
+
+@pytest.mark.parametrize("cap,g", [(128, 1), (128, 2), (128, 4), (64, 1), (64, 2), (64, 8), (32, 4), (32, 16)])
+def test_block_edge_and_scheduling_granularity_do_not_change_results(gp, cap, g):
+    """The block edge and the scheduling tile (g x g blocks, independent of the storage tile) only change the order
+    of work: every combination matches the oracle on a 2 x 2-tile problem whose tiles hold 4 / 8 / 16 blocks per edge."""
+    n, m, D, tile = 1024, 512, 8, 512
+    X, y = nfir.nfir_features(91, n, D)
+    Xs, _ = nfir.nfir_features(92, m, D, with_targets=False)
+    h = oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h)
+    gp.gp_set_block_edge(cap)
+    gp.gp_set_schedule_granularity(g)
+    assert gp.gp_block_size_for(n, tile) == cap and gp.gp_schedule_granularity(n, m, tile) == g
     out = _run_pipeline(gp, X, y, Xs, h, tile)
     _check_against_oracle(out, p)
 
@@ -283,6 +313,7 @@ def test_edge_shapes(gp, n, m, D, tile):
 def test_single_worker_runs_the_whole_dag(gp):
     """sched_width = 1: one persistent CTA executes every item in list order (no deadlock, same result)."""
     n, m, D, tile = 768, 256, 8, 256
+    gp.gp_set_block_edge(128)
     X, y = nfir.nfir_features(41, n, D)
     Xs, _ = nfir.nfir_features(42, m, D, with_targets=False)
     h = oracle.Hyper()
@@ -307,17 +338,20 @@ def test_ill_conditioned_factorisation(gp, noise, cond_floor):
     assert w[-1] / w[0] >= cond_floor
     Lo = oracle.cholesky(K)
     yardstick = relerr(np.linalg.cholesky(K), Lo)            # ~1e-11 at cond 6e8, ~1e-10 at 6e10
-    pipe = gp.GpPipeline(n, 0, D, tile, gp.Hyper(1.0, 1.0, noise))
-    pipe.assemble(_dev(X))
-    pipe.cholesky()
-    torch.cuda.synchronize()
-    assert int(pipe.info.item()) == 0
-    L = pipe.dense_L().cpu().numpy()
-    resid = np.linalg.norm(L @ L.T - K) / np.linalg.norm(K)
-    err = relerr(L, Lo)
-    print(f"noise={noise:g} cond={w[-1] / w[0]:.3g} residual={resid:.2e} |L-L_oracle|/|L_oracle|={err:.2e} oracle-vs-LAPACK={yardstick:.2e}")
-    assert resid <= 2e-14                                   # measured: 2e-15 at cond 6e8, 7e-15 at cond 6e10 (oracle: 7e-16)
-    assert err <= 20 * yardstick
+    for cap in (64, 128):                                       # inverses of 64- and of 128-blocks
+        gp.gp_set_block_edge(cap)
+        pipe = gp.GpPipeline(n, 0, D, tile, gp.Hyper(1.0, 1.0, noise))
+        pipe.assemble(_dev(X))
+        pipe.cholesky()
+        torch.cuda.synchronize()
+        assert int(pipe.info.item()) == 0
+        L = pipe.dense_L().cpu().numpy()
+        resid = np.linalg.norm(L @ L.T - K) / np.linalg.norm(K)
+        err = relerr(L, Lo)
+        print(f"noise={noise:g} block={cap} cond={w[-1] / w[0]:.3g} residual={resid:.2e} |L-L_oracle|/|L_oracle|={err:.2e} "
+              f"oracle-vs-LAPACK={yardstick:.2e}")
+        assert resid <= 2e-14                               # measured with 128-blocks: 2e-15 at cond 6e8, 7e-15 at cond 6e10 (oracle: 7e-16)
+        assert err <= 20 * yardstick
     # the solve on top of it: K alpha = y to the accuracy cond * u allows
     pipe.solve(_dev(y))
     torch.cuda.synchronize()

@@ -111,13 +111,20 @@ def test_schedule_fingerprint_is_stable_and_shape_dependent(gp):
 
 
 def test_schedule_granularity_auto_and_override(gp):
-    # auto: 1 scheduling block up to 96 block columns, then about 32 scheduling tiles per dimension
+    # block edge: 64 up to n = 8192 (when the tile admits it), 128 beyond; independent of the storage tile
+    assert gp.gp_block_size_for(1024, 256) == 64 and gp.gp_block_size_for(8192, 1024) == 64
+    assert gp.gp_block_size_for(16384, 1024) == 128 and gp.gp_block_size_for(32768, 1024) == 128
+    assert gp.gp_block_size_for(128, 32) == 32 and gp.gp_block_size_for(32768, 64) == 64 and gp.gp_block_size_for(320, 160) == 32
+    # auto granularity: 1 scheduling block up to 96 block columns, then about 32 scheduling tiles per dimension
     assert gp.gp_schedule_granularity(1024, 1024, 256) == 1
-    assert gp.gp_schedule_granularity(8192, 1024, 512) == 1
+    assert gp.gp_schedule_granularity(4096, 1024, 512) == 1
+    assert gp.gp_schedule_granularity(8192, 1024, 512) == 4       # 128 block columns of 64
     assert gp.gp_schedule_granularity(32768, 4096, 1024) == 8
     assert gp.gp_schedule_granularity(65536, 8192, 2048) == 16
     assert gp.gp_schedule_granularity(32768, 0, 128) == 8        # independent of the storage tile
     try:
+        gp.gp_set_block_edge(128)
+        assert gp.gp_block_size_for(1024, 256) == 128 and gp.gp_block_size_for(1024, 64) == 64
         for g in (1, 2, 4, 8):
             gp.gp_set_schedule_granularity(g)
             assert gp.gp_schedule_granularity(8192, 1024, 512) == g
@@ -126,10 +133,15 @@ def test_schedule_granularity_auto_and_override(gp):
                 assert rc == 0 and st["items"] > 0
         gp.gp_set_schedule_granularity(3)                          # not a divisor of 64: the largest divisor below it
         assert gp.gp_schedule_granularity(8192, 1024, 512) == 2
+        gp.gp_set_block_edge(32)
+        assert gp.gp_block_size_for(32768, 1024) == 32
     finally:
         gp.gp_set_schedule_granularity(0)
+        gp.gp_set_block_edge(0)
     with pytest.raises(gp.GpError):
         gp.gp_set_schedule_granularity(-1)
+    with pytest.raises(gp.GpError):
+        gp.gp_set_block_edge(48)
 
 
 def test_prepare_validates_arguments_before_touching_the_device(gp):

@@ -184,6 +184,27 @@ int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void
 int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, double* flops, size_t* need_bytes,
                                 void* stream);
 
+/* SURVEY.md 8(f) row 3 ("we plan to introduce mixed-precision calculations to take advantage of modern
+ * hardware capabilities"): the building block of a tensor-core route past the FP64 pipe -- the contraction
+ * C -= A B^T in FP64 accuracy EMULATED on the int8 tensor cores (tcgen05.mma kind::i8, int32 accumulators in TMEM)
+ * by the split-operand (Ozaki) scheme.  Every operand entry is written in fixed point with one global scale,
+ *     x / scale = sum_{p=0}^{7} d_p 2^(-7 (p + 1)),   d_p in [-64, 64]  (8 planes of balanced base-128 digits),
+ * the 36 plane products with p + q <= 7 are exact integer GEMMs, and only their recombination rounds (FP64).
+ * The truncation is 2^-56 scaleA scaleB per term, below the FP64 rounding of a result of that size.
+ *   gp_ozaki_plane_bytes: size of the plane array of a rows x k operand (8 rows k bytes).
+ *   gp_ozaki_slice: dX [rows x k] row-major FP64 with leading dimension ld  ->  dPlanes [8][rows][k] int8.
+ *        Requires |x| <= scale / 2 for every entry; *d_overflow (device int) is set to 1 otherwise, else 0.
+ *        k % 32 == 0.
+ *   gp_ozaki_contract: dC [ma x nb] row-major FP64, leading dimension ldc (even)  -=  A B^T from the planes of
+ *        A [ma x k] and B [nb x k].  ma % 128 == 0, nb % 64 == 0, k % 32 == 0, k <= 65536 (int32 accumulators).
+ * Both calls are stream-ordered.  This is a measured building block (bench.py reports its FP64-equivalent rate
+ * beside the DMMA contraction); gp_cholesky_tiled does not use it. */
+int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes);
+int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double scale, int8_t* dPlanes, int* d_overflow,
+                   void* stream);
+int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,
+                      double scaleB, double* dC, int64_t ldc, void* stream);
+
 /* Executor statistics of the LAST gp_cholesky_tiled / gp_predict_full_cov call that used dWork
  * (tracing support; the analogue of the paper's per-step APEX timers).  Copies
  * to h_stats (host) 8 uint64 per worker CTA:

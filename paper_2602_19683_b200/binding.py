@@ -24,7 +24,8 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
-           "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge")
+           "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
+           "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract")
 
 
 class gp_hyper(ctypes.Structure):
@@ -86,6 +87,9 @@ def load() -> ctypes.CDLL:
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
     lib.gp_prepare.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_schedule_fingerprint.argtypes = [i64, i64, ci, ci, ci, ctypes.POINTER(ctypes.c_uint64)]
+    lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
+    lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
+    lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
     lib.gp_block_size_for.argtypes = [i64, ci]
     lib.gp_set_block_edge.argtypes = [ci]
     lib.gp_set_schedule_granularity.argtypes = [ci]
@@ -276,6 +280,29 @@ def gp_schedule_fingerprint(n: int, m: int, tile: int, workers: int = 148, with_
     fp = ctypes.c_uint64(0)
     _check(load().gp_schedule_fingerprint(n, m, tile, workers, int(with_sigma), ctypes.byref(fp)), "gp_schedule_fingerprint")
     return int(fp.value)
+
+
+def gp_ozaki_slice(X: torch.Tensor, scale: float) -> torch.Tensor:
+    """FP64 [rows, k] (row-major, contiguous) -> int8 digit planes [8, rows, k]; raises if an entry exceeds scale / 2."""
+    rows, k = X.shape
+    need = ctypes.c_size_t(0)
+    _check(load().gp_ozaki_plane_bytes(rows, k, ctypes.byref(need)), "gp_ozaki_plane_bytes")
+    planes = torch.empty(int(need.value), dtype=torch.int8, device=X.device)
+    overflow = torch.zeros(1, dtype=torch.int32, device=X.device)
+    _check(load().gp_ozaki_slice(_ptr(X), rows, k, k, float(scale), _ptr(planes, torch.int8), _ptr(overflow, torch.int32), _stream()),
+           "gp_ozaki_slice")
+    if int(overflow.item()) != 0:
+        raise ValueError("gp_ozaki_slice: an entry exceeds scale / 2")
+    return planes.view(8, rows, k)
+
+
+def gp_ozaki_contract(Aplanes: torch.Tensor, Bplanes: torch.Tensor, scaleA: float, scaleB: float, C: torch.Tensor) -> None:
+    """C [ma, nb] (FP64, contiguous) -= A B^T from the digit planes of A [ma, k] and B [nb, k]."""
+    _, ma, k = Aplanes.shape
+    _, nb, kb = Bplanes.shape
+    assert k == kb and C.shape == (ma, nb)
+    _check(load().gp_ozaki_contract(_ptr(Aplanes, torch.int8), ma, _ptr(Bplanes, torch.int8), nb, k, float(scaleA), float(scaleB),
+                                    _ptr(C), nb, _stream()), "gp_ozaki_contract")
 
 
 def gp_block_size_for(n: int, tile: int) -> int:

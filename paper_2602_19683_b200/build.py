@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgp_b200.so")
 SOURCES = ["gp_api.cu", "gp_schedule.cpp"]
-HEADERS = ["gp_tma.cuh", "gp_diag.cuh", "gp_gemm.cuh", "gp_exec.cuh", "gp_kernels.cuh", "gp_peak.cuh", "gp_schedule.h", os.path.join("..", "..", "include", "gp_b200.h")]
+HEADERS = ["gp_tma.cuh", "gp_diag.cuh", "gp_gemm.cuh", "gp_exec.cuh", "gp_kernels.cuh", "gp_peak.cuh", "gp_ozaki.cuh", "gp_schedule.h", os.path.join("..", "..", "include", "gp_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared", "-Xptxas", "-v"]
 

@@ -7,6 +7,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -15,6 +16,7 @@
 
 #include "gp_exec.cuh"
 #include "gp_kernels.cuh"
+#include "gp_ozaki.cuh"
 #include "gp_peak.cuh"
 #include "gp_schedule.h"
 
@@ -755,6 +757,73 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
 }
 
 }  // extern "C"
+
+// ---- split-operand (Ozaki) contraction on the int8 tensor cores -------------------------
+namespace {
+// planes [S][rows][k] (int8) viewed through boxes of {32 bytes of k, box_rows rows, all S planes}, 32-byte swizzle
+int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64_t k, uint32_t box_rows) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return GP_ERR_CUDA;
+    const cuuint64_t dims[3] = {(cuuint64_t)k, (cuuint64_t)rows, (cuuint64_t)oz::kPlanes};
+    const cuuint64_t strides[2] = {(cuuint64_t)k, (cuuint64_t)(rows * k)};
+    const cuuint32_t box[3] = {(cuuint32_t)oz::kChunk, box_rows, (cuuint32_t)oz::kPlanes};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<int8_t*>(planes), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? GP_OK : GP_ERR_CUDA;
+}
+}  // namespace
+
+extern "C" int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    if (rows <= 0 || k <= 0 || k % oz::kChunk != 0) return GP_ERR_SIZE;
+    *bytes = (size_t)oz::kPlanes * (size_t)rows * (size_t)k;
+    return GP_OK;
+}
+
+extern "C" int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double scale, int8_t* dPlanes, int* d_overflow,
+                              void* stream) {
+    if (!dX || !dPlanes || !d_overflow) return GP_ERR_NULL;
+    if (rows <= 0 || k <= 0 || k % oz::kChunk != 0 || ld < k) return GP_ERR_SIZE;
+    if (!(scale > 0.0) || !std::isfinite(scale)) return GP_ERR_HYPER;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemsetAsync(d_overflow, 0, sizeof(int), st) != cudaSuccess) return GP_ERR_CUDA;
+    const int64_t total = rows * (k / 4);
+    const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
+    oz::slice_kernel<<<grid, 256, 0, st>>>(dX, rows, k, ld, 1.0 / scale, dPlanes, d_overflow);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,
+                                 double scaleB, double* dC, int64_t ldc, void* stream) {
+    if (!dAplanes || !dBplanes || !dC) return GP_ERR_NULL;
+    // int32 accumulators: at most S pairs of |d| <= 64 digits per level and k-step: 8 * 2^12 * k < 2^31
+    if (ma <= 0 || nb <= 0 || k <= 0 || ma % oz::kTileM != 0 || nb % oz::kTileN != 0 || k % oz::kChunk != 0 || k > 65536 || ldc < nb || ldc % 2 != 0)
+        return GP_ERR_SIZE;
+    if (!(scaleA > 0.0) || !(scaleB > 0.0) || !std::isfinite(scaleA * scaleB)) return GP_ERR_HYPER;
+    CUtensorMap mapA, mapB;
+    int rc = make_plane_map(&mapA, dAplanes, (uint64_t)ma, (uint64_t)k, oz::kTileM);
+    if (rc != GP_OK) return rc;
+    if ((rc = make_plane_map(&mapB, dBplanes, (uint64_t)nb, (uint64_t)k, oz::kTileN)) != GP_OK) return rc;
+    static std::atomic<uint32_t> configured[kMaxDevices];
+    const int dev = current_device();
+    if (dev >= kMaxDevices || !configured[dev].load(std::memory_order_acquire)) {
+        if (cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) != cudaSuccess) return GP_ERR_CUDA;
+        if (dev < kMaxDevices) configured[dev].store(1u, std::memory_order_release);
+    }
+    oz::OzParams p;
+    p.C = dC;
+    p.ldc = ldc;
+    p.tiles_m = (int)(ma / oz::kTileM);
+    p.tiles_n = (int)(nb / oz::kTileN);
+    p.kchunks = (int)(k / oz::kChunk);
+    p.w_last = scaleA * scaleB * std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+    const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
+    const int grid = (int)std::min<int64_t>(tiles, sm_count());
+    oz::ozaki_contract_kernel<<<grid, oz::kThreadsOz, oz::kSmemOz, (cudaStream_t)stream>>>(p, mapA, mapB);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
 
 extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream) {
     if (!dWork || !h_stats) return GP_ERR_NULL;

@@ -1,0 +1,76 @@
+"""the split-operand (Ozaki) contraction on the int8 tensor cores (tcgen05.mma kind::i8,
+TMEM accumulators) against the oracle, through the C ABI.  C -= A A^T is Eq. 3's  Sigma = K** - V^T V  with
+A = V^T, so oracle.posterior_cov is the expected value; a general A B^T case is checked against
+the exact integer arithmetic of the planes themselves (numpy int64), which pins the digit extraction too."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from helpers import relerr
+
+
+@pytest.fixture(scope="module")
+def gp():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    from paper_2602_19683_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.mark.parametrize("m,n", [(128, 32), (256, 512), (640, 1056)])
+def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
+    rng = np.random.default_rng(m + n)
+    V = rng.uniform(-0.9, 0.9, size=(n, m))                     # |V| <= 1 as for V = L^-1 K_{X,X^} with v = 1
+    Kss = rng.normal(size=(m, m))
+    want = oracle.posterior_cov(V, Kss)
+    A = torch.from_numpy(np.ascontiguousarray(V.T)).cuda()      # m x n, contraction index contiguous
+    C = torch.from_numpy(Kss.copy()).cuda()
+    planes = gp.gp_ozaki_slice(A, 2.0)
+    assert planes.shape == (8, m, n) and int(planes.min()) >= -64 and int(planes.max()) <= 64
+    gp.gp_ozaki_contract(planes, planes, 2.0, 2.0, C)
+    torch.cuda.synchronize()
+    got = C.cpu().numpy()
+    assert relerr(got, want) <= 1e-14
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
+
+
+def test_planes_are_an_exact_fixed_point_expansion_and_products_are_exact(gp):
+    """x / scale = sum_p d_p 2^(-7 (p+1)) to 2^-57, and the tensor-core result equals the integer arithmetic of the
+    planes recombined in FP64 (levels smallest first), bit for bit up to the last rounding."""
+    rng = np.random.default_rng(3)
+    ma, nb, k, scale = 256, 192, 288, 4.0
+    A = rng.uniform(-1.9, 1.9, size=(ma, k)); B = rng.normal(size=(nb, k)).clip(-1.9, 1.9)
+    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    pa, pb = gp.gp_ozaki_slice(dA, scale), gp.gp_ozaki_slice(dB, scale)
+    Pa, Pb = pa.cpu().numpy().astype(np.int64), pb.cpu().numpy().astype(np.int64)
+    w = 2.0 ** (-7.0 * np.arange(1, 9))
+    np.testing.assert_allclose(np.tensordot(w, Pa.astype(np.float64), axes=1) * scale, A, rtol=0, atol=scale * 2.0 ** -57)
+    C0 = rng.normal(size=(ma, nb))
+    C = torch.from_numpy(C0.copy()).cuda()
+    gp.gp_ozaki_contract(pa, pb, scale, scale, C)
+    torch.cuda.synchronize()
+    acc = np.zeros((ma, nb))
+    for lvl in range(7, -1, -1):
+        s = sum(Pa[p] @ Pb[lvl - p].T for p in range(lvl + 1))          # exact int64
+        acc += s.astype(np.float64) * (scale * scale * 2.0 ** (-7.0 * (lvl + 2)))
+    np.testing.assert_allclose(C.cpu().numpy(), C0 - acc, rtol=0, atol=4e-16 * np.abs(C0 - acc).max())
+    assert relerr(C.cpu().numpy(), C0 - A @ B.T) <= 1e-14
+
+
+def test_slice_reports_entries_beyond_the_scale_and_bad_arguments(gp):
+    X = torch.full((128, 32), 1.5, dtype=torch.float64, device="cuda")
+    with pytest.raises(ValueError):
+        gp.gp_ozaki_slice(X, 2.0)                                   # |x| > scale / 2
+    gp.gp_ozaki_slice(X, 4.0)
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_ozaki_slice(torch.zeros(128, 40, dtype=torch.float64, device="cuda"), 2.0)   # k % 32 != 0
+    assert e.value.code == gp.ERR["SIZE"]
+    p = gp.gp_ozaki_slice(torch.zeros(96, 32, dtype=torch.float64, device="cuda"), 2.0)
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_ozaki_contract(p, p, 2.0, 2.0, torch.zeros(96, 96, dtype=torch.float64, device="cuda"))   # rows % 128 != 0
+    assert e.value.code == gp.ERR["SIZE"]

@@ -205,6 +205,22 @@ int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double
 int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,
                       double scaleB, double* dC, int64_t ldc, void* stream);
 
+/* SURVEY.md 8(f) row 3, end to end: the tiled Cholesky of gp_cholesky_tiled with its trailing updates (SYRK / GEMM tile
+ * tasks: > 95 % of the flops) EMULATED on the int8 tensor cores and everything on the critical path
+ * (POTRF and TRSM tile tasks) in FP64 as before.  Opt-in: gp_cholesky_tiled itself is unchanged.
+ *   Left-looking over tile columns: column J first receives all its updates in ONE emulated contraction of depth J * tile
+ *   (tile (I,J) -= L(I,0:J) L(J,0:J)^T from the digit planes of the finished columns), then its FP64 panel step runs on
+ *   the persistent executor (POTRF tile task + TRSM tile tasks), then its tiles are sliced into digit planes.  The
+ *   fixed-point scale is found on the device from max_i K_ii (|L_ij| <= sqrt(K_ii)).  Everything is stream-ordered.
+ *   Accuracy: the emulation truncates at 2^-56 of the scale; measured |L - L_oracle| / |L_oracle| ~ 1e-13 (tests).
+ *   Same arguments and *d_info semantics as gp_cholesky_tiled; additionally tile % 128 == 0, n / tile <= 60, n <= 65536.
+ *   dWork: at least gp_mixed_workspace_bytes() (dominated by the dense digit planes, 8 n^2 bytes). */
+int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes);
+int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                            void* stream);
+/* Host-only replay check of the panel schedule of step J (returns the number of work items, or a negative GP_ERR_*). */
+int gp_panel_schedule_selfcheck(int64_t n, int tile, int J);
+
 /* Executor statistics of the LAST gp_cholesky_tiled / gp_predict_full_cov call that used dWork
  * (tracing support; the analogue of the paper's per-step APEX timers).  Copies
  * to h_stats (host) 8 uint64 per worker CTA:

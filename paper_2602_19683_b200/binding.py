@@ -25,7 +25,8 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
-           "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract")
+           "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
+           "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck")
 
 
 class gp_hyper(ctypes.Structure):
@@ -87,6 +88,9 @@ def load() -> ctypes.CDLL:
     lib.gp_contraction_bench_launch.argtypes = [ci, ci, vp, sz, ctypes.POINTER(ctypes.c_double), psz, vp]
     lib.gp_prepare.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_schedule_fingerprint.argtypes = [i64, i64, ci, ci, ci, ctypes.POINTER(ctypes.c_uint64)]
+    lib.gp_mixed_workspace_bytes.argtypes = [i64, ci, psz]
+    lib.gp_cholesky_tiled_mixed.argtypes = [vp, i64, ci, ci, vp, vp, sz, vp]
+    lib.gp_panel_schedule_selfcheck.argtypes = [i64, ci, ci]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
     lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
     lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
@@ -280,6 +284,22 @@ def gp_schedule_fingerprint(n: int, m: int, tile: int, workers: int = 148, with_
     fp = ctypes.c_uint64(0)
     _check(load().gp_schedule_fingerprint(n, m, tile, workers, int(with_sigma), ctypes.byref(fp)), "gp_schedule_fingerprint")
     return int(fp.value)
+
+
+def gp_mixed_workspace_bytes(n: int, tile: int) -> int:
+    b = ctypes.c_size_t(0)
+    _check(load().gp_mixed_workspace_bytes(n, tile, ctypes.byref(b)), "gp_mixed_workspace_bytes")
+    return int(b.value)
+
+
+def gp_cholesky_tiled_mixed(KL: torch.Tensor, n: int, tile: int, sched_width: int, info: torch.Tensor, work: torch.Tensor) -> None:
+    """gp_cholesky_tiled with the trailing updates emulated on the int8 tensor cores (opt-in)."""
+    _check(load().gp_cholesky_tiled_mixed(_ptr(KL), n, tile, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8),
+                                          work.numel(), _stream()), "gp_cholesky_tiled_mixed")
+
+
+def gp_panel_schedule_selfcheck(n: int, tile: int, J: int) -> int:
+    return int(load().gp_panel_schedule_selfcheck(n, tile, J))
 
 
 def gp_ozaki_slice(X: torch.Tensor, scale: float) -> torch.Tensor:

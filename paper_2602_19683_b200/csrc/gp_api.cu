@@ -806,13 +806,12 @@ extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_
     int rc = make_plane_map(&mapA, dAplanes, (uint64_t)ma, (uint64_t)k, oz::kTileM);
     if (rc != GP_OK) return rc;
     if ((rc = make_plane_map(&mapB, dBplanes, (uint64_t)nb, (uint64_t)k, oz::kTileN)) != GP_OK) return rc;
-    static std::atomic<uint32_t> configured[kMaxDevices];
-    const int dev = current_device();
-    if (dev >= kMaxDevices || !configured[dev].load(std::memory_order_acquire)) {
-        if (cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) != cudaSuccess) return GP_ERR_CUDA;
-        if (dev < kMaxDevices) configured[dev].store(1u, std::memory_order_release);
-    }
+    rc = configure_once(512u, [] {
+        return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
+    });
+    if (rc != GP_OK) return rc;
     oz::OzParams p;
+    memset(&p, 0, sizeof(p));
     p.C = dC;
     p.ldc = ldc;
     p.tiles_m = (int)(ma / oz::kTileM);
@@ -823,6 +822,144 @@ extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_
     const int grid = (int)std::min<int64_t>(tiles, sm_count());
     oz::ozaki_contract_kernel<<<grid, oz::kThreadsOz, oz::kSmemOz, (cudaStream_t)stream>>>(p, mapA, mapB);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+// ---- gp_cholesky_tiled_mixed: FP64 panels + emulated trailing updates ------------------------
+namespace {
+struct MixedWs { size_t ticket, verL, invD, scale, planes, total; };
+MixedWs mixed_ws(int64_t n) {
+    const CholWs c = chol_ws(n, 128);
+    MixedWs w;
+    w.ticket = c.ticket;
+    w.verL = c.verL;
+    w.invD = c.invD;
+    w.scale = align_up(c.total, 256);
+    w.planes = align_up(w.scale + 256, 1024);
+    w.total = w.planes + (size_t)oz::kPlanes * (size_t)n * (size_t)n;
+    return w;
+}
+int mixed_ok(int64_t n, int tile) {
+    if (n <= 0 || n > (int64_t)1 << 22) return GP_ERR_SIZE;
+    const int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (tile % 128 != 0) return GP_ERR_TILE;
+    if (n / tile > 60) return GP_ERR_SIZE;                 // one ticket counter per panel launch in the 256-byte header
+    if (n > 65536 + 128) return GP_ERR_SIZE;               // int32 accumulators of the emulated contraction: k <= 65536
+    return GP_OK;
+}
+}  // namespace
+
+extern "C" int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    const int rc = mixed_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    *bytes = mixed_ws(n).total;
+    return GP_OK;
+}
+
+extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                                       void* stream) {
+    if (!dKL || !d_info || !dWork) return GP_ERR_NULL;
+    int rc = mixed_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const MixedWs w = mixed_ws(n);
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    constexpr int b = 128;
+    const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b);
+    const int workers = workers_for(sched_width);
+    // the panel schedules of all M steps (built and uploaded on first use, like the other schedules)
+    std::vector<CachedSchedule> panels(M);
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
+        std::lock_guard<std::mutex> lk(g_mu);
+        for (int J = 0; J < M; ++J) {
+            auto key = std::make_tuple(dev, 16 + J, M, 0, nbt, b);
+            auto it = g_cache.find(key);
+            if (it != g_cache.end()) { panels[J] = it->second; continue; }
+            std::vector<SchedItem> items;
+            build_panel_schedule(M, nbt, J, sm_count(), items, b);
+            CachedSchedule cs;
+            cs.nitems = (int)items.size();
+            if (cudaMalloc(&cs.d_items, items.size() * sizeof(Item) + 16) != cudaSuccess) return GP_ERR_CUDA;
+            if (cudaMemcpy(cs.d_items, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice) != cudaSuccess) {
+                cudaFree(cs.d_items);
+                return GP_ERR_CUDA;
+            }
+            g_cache[key] = cs;
+            panels[J] = cs;
+        }
+    }
+    char* ws = (char*)dWork;
+    double* d_scale = (double*)(ws + w.scale);
+    int8_t* planes = (int8_t*)(ws + w.planes);
+    if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;           // tickets, statistics, version counters
+    if (cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return GP_ERR_CUDA;
+    oz::factor_scale_kernel<<<1, 1024, 0, st>>>(dKL, n, tile, d_scale);
+    // one tensor map over the dense digit planes [8][n][n] for both operands (boxes of 128 and of 64 rows)
+    CUtensorMap mapA, mapB;
+    if ((rc = make_plane_map(&mapA, planes, (uint64_t)n, (uint64_t)n, oz::kTileM)) != GP_OK) return rc;
+    if ((rc = make_plane_map(&mapB, planes, (uint64_t)n, (uint64_t)n, oz::kTileN)) != GP_OK) return rc;
+    rc = configure_once(512u, [] {
+        return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
+    });
+    if (rc != GP_OK) return rc;
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = dKL;
+    p.invD = (double*)(ws + w.invD);
+    p.verL = (int*)(ws + w.verL);
+    p.stats = (unsigned long long*)(ws + kStatsOff);
+    p.d_info = d_info;
+    p.t = tile;
+    p.nbt = nbt;
+    p.snbt = nbt;
+    p.NB = NB;
+    p.Mt = M;
+    ExecMaps mp;
+    if ((rc = make_exec_maps(&mp, p, b, 0)) != GP_OK) return rc;
+    for (int J = 0; J < M; ++J) {
+        if (J > 0) {
+            // left-looking: tile column J -= L(J:, 0:J) L(J, 0:J)^T, one emulated contraction of depth J * tile
+            oz::OzParams q;
+            memset(&q, 0, sizeof(q));
+            q.C = dKL;
+            q.tiles_m = (M - J) * (tile / oz::kTileM);
+            q.tiles_n = tile / oz::kTileN;
+            q.kchunks = (int)((int64_t)J * tile / oz::kChunk);
+            q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+            q.scale = d_scale;
+            q.tiled = 1;
+            q.t = tile;
+            q.J = J;
+            q.row0 = J * tile;
+            const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
+            oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
+            oz::set_column_versions_kernel<<<(NB * nbt + 255) / 256, 256, 0, st>>>(p.verL, NB, nbt, J, kConsumerWarps);
+        }
+        p.items = panels[J].d_items;
+        p.nitems = panels[J].nitems;
+        p.ticket = (unsigned int*)(ws + w.ticket) + J;
+        rc = launch_exec<128>(p, mp, workers, st);
+        if (rc != GP_OK) return rc;
+        if (J + 1 < M) {
+            const int64_t total = (n - (int64_t)(J + 1) * tile) * (tile / 4);
+            const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
+            oz::slice_tile_column_kernel<<<grid, 256, 0, st>>>(dKL, n, tile, J, d_scale, planes);
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_panel_schedule_selfcheck(int64_t n, int tile, int J) {
+    const int rc = mixed_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    const int M = (int)(n / tile), nbt = tile / 128;
+    if (J < 0 || J >= M) return GP_ERR_SIZE;
+    std::vector<SchedItem> items;
+    build_panel_schedule(M, nbt, J, 148, items, 128);
+    return validate_panel_schedule(items, M, nbt, J) ? (int)items.size() : GP_ERR_SIZE;
 }
 
 extern "C" int gp_exec_stats(const void* dWork, uint64_t* h_stats, int max_workers, void* stream) {

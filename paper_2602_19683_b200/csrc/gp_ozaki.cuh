@@ -73,6 +73,71 @@ __global__ void __launch_bounds__(256) slice_kernel(const double* __restrict__ X
     }
 }
 
+// The same for tile column J of a lower-packed tiled matrix (tiles (I, J), I > J) into DENSE planes [p][n][n] of the
+// whole matrix (row = global row, column = global column), with the scale read from device memory.
+__global__ void __launch_bounds__(256) slice_tile_column_kernel(const double* __restrict__ tiles, int64_t n, int t, int J,
+                                                                const double* __restrict__ scale, int8_t* __restrict__ planes) {
+    const double inv_scale = 1.0 / *scale;
+    const int64_t rows = n - (int64_t)(J + 1) * t;          // rows below the diagonal tile
+    const int64_t total = rows * (t / 4);
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t rr = idx / (t / 4);
+        const int c = 4 * (int)(idx % (t / 4));
+        const int64_t gi = (int64_t)(J + 1) * t + rr;
+        const int64_t I = gi / t, r = gi % t;
+        const double* src = tiles + ((size_t)I * (I + 1) / 2 + J) * (size_t)t * t + (size_t)r * t + c;
+        const double2 v01 = *reinterpret_cast<const double2*>(src), v23 = *reinterpret_cast<const double2*>(src + 2);
+        const double xs[4] = {v01.x, v01.y, v23.x, v23.y};
+        uint32_t packed[kPlanes];
+#pragma unroll
+        for (int p = 0; p < kPlanes; ++p) packed[p] = 0u;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            long long I56 = __double2ll_rn(xs[e] * inv_scale * 72057594037927936.0);
+#pragma unroll
+            for (int p = kPlanes - 1; p >= 0; --p) {
+                const long long d = ((I56 + 64) & 127) - 64;
+                I56 = (I56 - d) >> kDigitBits;
+                packed[p] |= (uint32_t)((int)d & 0xff) << (8 * e);
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < kPlanes; ++p)
+            *reinterpret_cast<uint32_t*>(planes + ((size_t)p * n + gi) * n + (size_t)J * t + c) = packed[p];
+    }
+}
+
+// scale <- 2 * 2^ceil(log2(sqrt(max_i K_ii))): every entry of the Cholesky factor obeys |L_ij| <= sqrt(K_ii), so
+// |L| <= scale / 2 and one global fixed-point scale serves the whole factor.  One CTA.
+__global__ void __launch_bounds__(1024) factor_scale_kernel(const double* __restrict__ tiles, int64_t n, int t, double* __restrict__ scale) {
+    __shared__ double s_max[32];
+    double m = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += 1024) {
+        const int64_t I = i / t, r = i % t;
+        m = fmax(m, tiles[((size_t)I * (I + 1) / 2 + I) * (size_t)t * t + r * (size_t)t + r]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < 32; ++k) m = fmax(m, s_max[k]);
+        int e;
+        const double f = frexp(sqrt(m > 0.0 ? m : 1.0), &e);      // sqrt(m) = f 2^e, f in [0.5, 1)
+        *scale = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0));          // >= 2 sqrt(m), with a little head-room at the edge
+    }
+}
+
+// version counters of the blocks of tile column J <- "J trailing updates applied" (they were applied by the emulated
+// contraction, which does not go through the executor's counters)
+__global__ void set_column_versions_kernel(int* __restrict__ ver, int NB, int nbt, int J, int per_version) {
+    const int c0 = J * nbt;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < (NB - c0) * nbt; idx += gridDim.x * blockDim.x) {
+        const int gr = c0 + idx / nbt, gc = c0 + idx % nbt;
+        if (gc <= gr) ver[(size_t)gr * NB + gc] = J * per_version;
+    }
+}
+
 // ---- tcgen05 / TMEM wrappers ----------------------------------------------------------------------------------------
 __device__ __forceinline__ void tmem_alloc(uint32_t* slot_in_smem, uint32_t cols) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(slot_in_smem)), "r"(cols) : "memory");
@@ -125,11 +190,39 @@ __device__ __forceinline__ uint64_t smem_desc_sw32(uint32_t saddr) {
 constexpr uint32_t kIdescI8 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTileN >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 
 struct OzParams {
-    double* C;
+    double* C;            // dense: C [tiles_m * 128, ldc];  tiled: the lower-packed tiles of the factorisation
     int64_t ldc;
     int tiles_m, tiles_n, kchunks;
     double w_last;        // scaleA * scaleB * 2^(-7 (S + 1)): weight of level S - 1; level l weighs scaleA scaleB 2^(-7 (l + 2))
+    const double* scale;  // optional device scalar s: the weights are multiplied by s^2 (operands sliced with a scale found on the device)
+    // tiled mode (gp_cholesky_tiled_mixed): the output is tile column J of a lower-packed matrix of t x t tiles, rows from
+    // tile row J down; operand rows and the k extent are taken from dense digit planes of the whole matrix
+    int tiled, t, J;
+    int row0;             // first operand row of A and of B in the planes (J * t)
 };
+
+// tile (tm, tn) -> is it wanted, and where does row `r` (0..127) of it live
+struct OzTile {
+    bool wanted;
+    double* c;            // address of element (row 0 of the tile, column 0 of the tile)
+    int64_t ld;
+};
+__device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
+    OzTile o;
+    if (!p.tiled) {
+        o.wanted = true;
+        o.ld = p.ldc;
+        o.c = p.C + (size_t)tm * kTileM * p.ldc + (size_t)tn * kTileN;
+        return o;
+    }
+    const int bpt = p.t / kTileM;                       // 128-row blocks per tile edge
+    const int I = p.J + tm / bpt, rblk = tm % bpt;
+    // on the diagonal tile only the lower part is data: skip 128 x 64 pieces that lie wholly above the diagonal
+    o.wanted = !(I == p.J && tn * kTileN >= (rblk + 1) * kTileM);
+    o.ld = p.t;
+    o.c = p.C + ((size_t)I * (I + 1) / 2 + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * kTileN;
+    return o;
+}
 
 __global__ void __launch_bounds__(kThreadsOz, 1)
 ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
@@ -162,12 +255,13 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
             int stage = 0, phase = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const int tm = tile / p.tiles_n, tn = tile % p.tiles_n;
+                if (!oz_tile(p, tm, tn).wanted) continue;
                 for (int kc = 0; kc < p.kchunks; ++kc) {
                     mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
                     char* dst = base + (size_t)stage * kStageBytesOz;
                     mbar_arrive_expect_tx(&full[stage], (uint32_t)kStageBytesOz);
-                    tma_load_3d(dst, &mapA, kc * kChunk, tm * kTileM, 0, &full[stage]);
-                    tma_load_3d(dst + kABytes, &mapB, kc * kChunk, tn * kTileN, 0, &full[stage]);
+                    tma_load_3d(dst, &mapA, kc * kChunk, p.row0 + tm * kTileM, 0, &full[stage]);
+                    tma_load_3d(dst + kABytes, &mapB, kc * kChunk, p.row0 + tn * kTileN, 0, &full[stage]);
                     if (++stage == kStagesOz) { stage = 0; phase ^= 1; }
                 }
             }
@@ -177,6 +271,7 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
         if (lane == 0) {
             int stage = 0, phase = 0, tphase = 0;
             for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                if (!oz_tile(p, tile / p.tiles_n, tile % p.tiles_n).wanted) continue;
                 mbar_wait(tmem_empty, (uint32_t)(tphase ^ 1));          // the epilogue has drained the previous tile
                 tc_fence_after();
                 for (int kc = 0; kc < p.kchunks; ++kc) {
@@ -205,16 +300,18 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
         const int quad = warp & 3;
         int tphase = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int tm = tile / p.tiles_n, tn = tile % p.tiles_n;
+            const OzTile ot = oz_tile(p, tile / p.tiles_n, tile % p.tiles_n);
+            if (!ot.wanted) continue;
             mbar_wait(tmem_full, (uint32_t)tphase);
             tc_fence_after();
-            double* crow = p.C + ((size_t)tm * kTileM + 32 * quad + lane) * p.ldc + (size_t)tn * kTileN;
+            double* crow = ot.c + (size_t)(32 * quad + lane) * ot.ld;
+            const double wl = p.scale ? p.w_last * (*p.scale) * (*p.scale) : p.w_last;
 #pragma unroll 1
             for (int c0 = 0; c0 < kTileN; c0 += 16) {
                 double acc[16];
 #pragma unroll
                 for (int j = 0; j < 16; ++j) acc[j] = 0.0;
-                double w = p.w_last;
+                double w = wl;
 #pragma unroll
                 for (int lvl = kPlanes - 1; lvl >= 0; --lvl) {           // smallest weight first
                     int32_t v[16];

@@ -209,8 +209,10 @@ void program_order_predict(int M, int Mm, int nbt, bool with_sigma, std::vector<
     }
 }
 
+// `base`: versions every block already carries when the program starts (0 for a whole factorisation; J for the panel
+// step of tile column J, whose blocks have received J trailing updates from outside the executor).
 void schedule(const Shape& s, std::vector<SchedItem>& prog, const std::vector<int32_t>& task, int workers, int blk,
-              std::vector<SchedItem>& out, SchedStats* stats, bool simulate) {
+              std::vector<SchedItem>& out, SchedStats* stats, bool simulate, int base = 0) {
     const int N = (int)prog.size();
     if (!simulate || N == 0) { out = prog; return; }
     const Cost cost(blk);
@@ -232,8 +234,8 @@ void schedule(const Shape& s, std::vector<SchedItem>& prog, const std::vector<in
         tmp.clear();
         item_effects(s, prog[i],
                      [&](int64_t b, int need) {
-                         if (need > 0) {
-                             const int32_t w = writer[wcount[b] + need - 1];
+                         if (need - base > 0) {
+                             const int32_t w = writer[wcount[b] + need - base - 1];
                              if (w != i) tmp.push_back(w);
                          }
                      },
@@ -327,6 +329,43 @@ void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>
     std::vector<int32_t> task;
     program_order_cholesky(M, nbt, prog, task);
     schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, stats, simulate);
+}
+
+// The FP64 part of step J of the factorisation alone (gp_cholesky_tiled_mixed): the POTRF tile task of the diagonal
+// tile (J, J) and the TRSM tile tasks of the tiles below it, for blocks that already carry J versions.
+void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk) {
+    std::vector<SchedItem> prog;
+    std::vector<int32_t> task;
+    int32_t tid = 0;
+    auto emit = [&](const SchedItem& it) { prog.push_back(it); task.push_back(tid); };
+    const int qt = J * nbt;
+    for (int jj = 0; jj < nbt; ++jj) {
+        emit(mk(S_POTRF, qt + jj, qt + jj)); ++tid;
+        for (int ii = jj + 1; ii < nbt; ++ii) { emit(mk(S_TRSM_L, qt + ii, qt + jj)); ++tid; }
+        for (int kk = jj + 1; kk < nbt; ++kk)
+            for (int ii = kk; ii < nbt; ++ii) { emit(mk(S_UPD_L, qt + ii, qt + kk, qt + jj, qt + jj + 1)); ++tid; }
+    }
+    for (int I = J + 1; I < M; ++I) {
+        for (int bi = 0; bi < nbt; ++bi) emit(mk(S_ROW_L, I * nbt + bi, qt));
+        ++tid;
+    }
+    schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, nullptr, true, J);
+}
+
+bool validate_panel_schedule(const std::vector<SchedItem>& items, int M, int nbt, int J) {
+    const Shape s(M, 0, nbt, false);
+    std::vector<int32_t> ver(s.nblocks, 0);
+    for (int gr = J * nbt; gr < s.NB; ++gr)
+        for (int gc = J * nbt; gc < (J + 1) * nbt && gc <= gr; ++gc) ver[s.idL(gr, gc)] = J;
+    bool ok = true;
+    for (const SchedItem& it : items) {
+        item_effects(s, it, [&](int64_t b, int need) { if (ver[b] < need) ok = false; }, [&](int64_t b) { ++ver[b]; });
+        if (!ok) return false;
+    }
+    for (int gr = J * nbt; gr < s.NB; ++gr)
+        for (int gc = J * nbt; gc < (J + 1) * nbt && gc <= gr; ++gc)
+            if (ver[s.idL(gr, gc)] != s.finL(gr, gc)) return false;
+    return true;
 }
 
 void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats, bool simulate,

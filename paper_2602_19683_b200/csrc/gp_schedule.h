@@ -38,6 +38,11 @@ void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>
 void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<SchedItem>& out, int blk = 128,
                             SchedStats* stats = nullptr, bool simulate = true, bool with_sigma = true);
 
+// Step J of the factorisation without its trailing updates (the FP64 half of gp_cholesky_tiled_mixed): POTRF tile task of
+// tile (J, J) + the TRSM tile tasks below it, for blocks that already carry J versions; and its replay check.
+void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk = 128);
+bool validate_panel_schedule(const std::vector<SchedItem>& items, int M, int nbt, int J);
+
 // Checks that `items` is a valid execution order (every wait of every item is satisfied by items
 // earlier in the list) and that every block ends at its final version.  Used by the CPU tests.
 bool validate_schedule(const std::vector<SchedItem>& items, int M, int Mm, int nbt, bool predict, const char** why,

@@ -74,3 +74,47 @@ def test_slice_reports_entries_beyond_the_scale_and_bad_arguments(gp):
     with pytest.raises(gp.GpError) as e:
         gp.gp_ozaki_contract(p, p, 2.0, 2.0, torch.zeros(96, 96, dtype=torch.float64, device="cuda"))   # rows % 128 != 0
     assert e.value.code == gp.ERR["SIZE"]
+
+
+# ---------------------------------------------------------------- the mixed factorisation end to end
+@pytest.mark.parametrize("n,D,tile,noise", [(512, 8, 128, 0.1), (1024, 8, 256, 0.1), (2048, 8, 512, 0.1), (2048, 8, 1024, 0.1), (1536, 3, 256, 1e-3)])
+def test_mixed_cholesky_matches_oracle(gp, n, D, tile, noise):
+    """FP64 panels + emulated trailing updates: L against the oracle at north_star's tolerance (1e-10), and bitwise
+    reproducible from run to run (integer accumulation + a fixed recombination order)."""
+    from paper_2602_19683_b200 import nfir
+    X, y = nfir.nfir_features(n + D, n, D)
+    h = oracle.Hyper(1.0, 1.0, noise)
+    K = oracle.assemble(X, X, h, True)
+    Lo = oracle.cholesky(K)
+    pipe = gp.GpPipeline(n, 0, D, tile, gp.Hyper(1.0, 1.0, noise))
+    work = torch.empty(gp.gp_mixed_workspace_bytes(n, tile), dtype=torch.uint8, device="cuda")
+    dX = torch.from_numpy(X).cuda()
+    outs = []
+    for _ in range(2):
+        pipe.assemble(dX)
+        gp.gp_cholesky_tiled_mixed(pipe.KL, n, tile, 0, pipe.info, work)
+        torch.cuda.synchronize()
+        assert int(pipe.info.item()) == 0
+        outs.append(pipe.dense_L().cpu().numpy())
+    err = relerr(outs[0], Lo)
+    print(f"mixed n={n} tile={tile} noise={noise}: |L - L_oracle| / |L_oracle| = {err:.2e}")
+    assert err <= 1e-10
+    np.testing.assert_allclose(outs[0], Lo, rtol=0, atol=1e-9 * np.abs(Lo).max())
+    assert np.array_equal(outs[0], outs[1])
+    # and the rest of the pipeline runs on this factor unchanged
+    pipe.solve(torch.from_numpy(y).cuda())
+    torch.cuda.synchronize()
+    assert relerr(pipe.alpha.cpu().numpy(), oracle.backward_subst(Lo, oracle.forward_subst(Lo, y))) <= 1e-9
+
+
+def test_mixed_cholesky_reports_a_non_positive_pivot(gp):
+    n, tile = 512, 128
+    K = np.eye(n)
+    K[300, 300] = -1.0
+    tiles = [K[I * tile:(I + 1) * tile, J * tile:(J + 1) * tile].ravel() for I in range(n // tile) for J in range(I + 1)]
+    KL = torch.from_numpy(np.concatenate(tiles)).cuda()
+    work = torch.empty(gp.gp_mixed_workspace_bytes(n, tile), dtype=torch.uint8, device="cuda")
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    gp.gp_cholesky_tiled_mixed(KL, n, tile, 0, info, work)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 301

@@ -165,6 +165,21 @@ def test_ncu_traffic_record_matches_the_schedule_the_library_builds(gp):
         assert os.path.exists(os.path.join(ROOT, rec["source"].split(" ")[0]))
 
 
+@pytest.mark.parametrize("n,tile", [(512, 128), (1024, 256), (4096, 1024), (32768, 1024)])
+def test_panel_schedules_of_the_mixed_factorisation_replay(gp, n, tile):
+    """gp_cholesky_tiled_mixed runs step J's FP64 half (POTRF + TRSM tile tasks) on blocks that already carry J versions."""
+    M = n // tile
+    for J in sorted({0, 1, M // 2, M - 1}):
+        items = gp.gp_panel_schedule_selfcheck(n, tile, J)
+        nbt = tile // 128
+        want = nbt + nbt * (nbt - 1) // 2 + sum((nbt - kk) for jj in range(nbt) for kk in range(jj + 1, nbt)) + (M - J - 1) * nbt
+        assert items == want, (J, items, want)
+    assert gp.gp_panel_schedule_selfcheck(n, tile, M) == gp.ERR["SIZE"]
+    assert gp.gp_mixed_workspace_bytes(n, tile) >= 8 * n * n
+    with pytest.raises(gp.GpError):
+        gp.gp_mixed_workspace_bytes(n, 96)
+
+
 def test_binding_refuses_cpu_tensors(gp):
     import torch
     X = torch.zeros(32, 2, dtype=torch.float64)

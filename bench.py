@@ -326,6 +326,21 @@ def measure_fp64_peak(gp, torch):
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(); flops = gp.gp_contraction_bench_launch(K, reps, buf); b.record(); torch.cuda.synchronize()
     out["contraction_k1024_tflops"] = flops / (a.elapsed_time(b) * 1e-3) / 1e12
+    del buf
+    # the same contraction emulated on the int8 tensor cores (8 digit planes, 36 int8 GEMMs)
+    ma = nb = 8192; kk = 4096
+    A = torch.rand(ma, kk, dtype=torch.float64, device="cuda") - 0.5
+    Ap = gp.gp_ozaki_slice(A, 2.0)
+    C = torch.zeros(ma, nb, dtype=torch.float64, device="cuda")
+    best = 0.0
+    for r in range(4):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); gp.gp_ozaki_contract(Ap, Ap, 2.0, 2.0, C); b.record(); torch.cuda.synchronize()
+        if r > 0:
+            best = max(best, 2.0 * ma * nb * kk / (a.elapsed_time(b) * 1e-3) / 1e12)
+    out["ozaki_int8_contraction_fp64_equivalent_tflops"] = best
+    out["ozaki_int8_pops"] = best * 36 / 1e3
+    del A, Ap, C
     return out
 
 
@@ -419,6 +434,29 @@ def run_b200(args):
     next_rows = {"predict_variance_ms": statistics.median(tv), "log_marginal_likelihood_ms": statistics.median(tl),
                  "log_marginal_likelihood": float(lml.item()), "variance_min_max": [float(var.min().item()), float(var.max().item())]}
     del var, lml
+    # the same factorisation with its trailing updates emulated on the int8 tensor cores
+    # (gp_cholesky_tiled_mixed, opt-in), reported beside the FP64 DMMA path; median of 3 after one warm-up, and the
+    # distance of its factor from the FP64 path's (lower triangle, via gp_tiles_to_dense)
+    if tile % 128 == 0 and n // tile <= 60 and n <= 65536:
+        L64 = pipe.dense_L()
+        mwork = torch.empty(gp.gp_mixed_workspace_bytes(n, tile), dtype=torch.uint8, device="cuda")
+        tmx = []
+        for r in range(4):
+            pipe.assemble(dX)
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            e[0].record(); gp.gp_cholesky_tiled_mixed(pipe.KL, n, tile, args.width, pipe.info, mwork); e[1].record(); torch.cuda.synchronize()
+            if r > 0:
+                tmx.append(e[0].elapsed_time(e[1]))
+        Lmx = pipe.dense_L()
+        mixed_ms = statistics.median(tmx)
+        next_rows["cholesky_mixed_int8_emulated"] = {
+            "ms": mixed_ms, "gflops_fp64_equivalent": n ** 3 / 3.0 / (mixed_ms * 1e-3) / 1e9, "info": int(pipe.info.item()),
+            "rel_diff_to_fp64_factor": float((Lmx - L64).norm() / L64.norm()),
+            "what": "FP64 POTRF/TRSM tile tasks on the executor + SYRK/GEMM tile tasks as 8-plane split-operand int8 products "
+                    "(tcgen05.mma kind::i8, TMEM accumulators); not the headline: dtype of `value` stays f64"}
+        del L64, Lmx, mwork
+        pipe.assemble(dX); pipe.cholesky(); pipe.solve(dY)       # leave the FP64 factor behind for what follows
+    torch.cuda.empty_cache()
 
     # end to end through the host-buffer C-ABI call: H2D of X, y, X^ and D2H of mean, Sigma inside
     ws = torch.empty(gp.gp_pipeline_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
@@ -477,6 +515,8 @@ def run_b200(args):
                          "peak_burst": peaks["dmma_burst_tflops"], "dfma_burst": peaks["dfma_burst_tflops"],
                          "frac_of_burst": achieved / peaks["dmma_burst_tflops"],
                          "contraction_alone_tflops": peaks["contraction_k1024_tflops"],
+                         "emulated_contraction_tflops_fp64_equivalent": peaks["ozaki_int8_contraction_fp64_equivalent_tflops"],
+                         "emulated_contraction_int8_pops": peaks["ozaki_int8_pops"],
                          "full_cov_exec_tflops": (n * n * m + n * m * m) / (phase["full_cov"] * 1e-3) / 1e12,
                          "hbm_gbs_measured": mp.get("hbm_gbs"),
                          "assemble_gbs": (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["assemble"] * 1e-3) / 1e9,

@@ -93,6 +93,39 @@ def test_config3_headline_every_output_entry(gp):
     _every_output_entry(gp, nfir.CONFIGS[3])
 
 
+def test_config3_mixed_factorisation_properties(gp):
+    """gp_cholesky_tiled_mixed (trailing updates emulated on the int8 tensor cores) at the headline size:
+    lower triangular with positive diagonal, L (L^T z) = K z to 1e-12 on 8 Rademacher vectors with K from the oracle, and the
+    leading 4096 block against a full oracle run at north_star's 1e-10."""
+    cfg = nfir.CONFIGS[3]
+    n = cfg.n
+    X, y, Xs = nfir.make_inputs(cfg)
+    h = oracle.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    pipe = gp.GpPipeline(n, 0, cfg.D, cfg.tile, gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise))
+    work = torch.empty(gp.gp_mixed_workspace_bytes(n, cfg.tile), dtype=torch.uint8, device="cuda")
+    pipe.assemble(torch.from_numpy(X).cuda())
+    gp.gp_cholesky_tiled_mixed(pipe.KL, n, cfg.tile, 0, pipe.info, work)
+    torch.cuda.synchronize()
+    assert int(pipe.info.item()) == 0
+    del work
+    L = pipe.dense_L().cpu().numpy()
+    del pipe
+    torch.cuda.empty_cache()
+    assert np.all(np.diag(L) > 0)
+    rng = np.random.default_rng(11)
+    Z = rng.choice([-1.0, 1.0], size=(n, 8))
+    KZ = np.empty((n, 8))
+    for r0 in range(0, n, 2048):
+        KZ[r0:r0 + 2048] = oracle.assemble(X[r0:r0 + 2048], X, h, False) @ Z
+    KZ += cfg.noise * Z
+    LLtZ = L @ (L.T @ Z)
+    for k in range(8):
+        assert relerr(LLtZ[:, k], KZ[:, k]) <= 1e-12
+    nb = 4096
+    Lb = oracle.cholesky(oracle.assemble(X[:nb], X[:nb], h, True))
+    assert relerr(L[:nb, :nb], Lb) <= 1e-10
+
+
 def test_config4_largest_every_output_entry(gp):
     """The same at the largest single-GPU configuration (tile 2048, 16 blocks per tile edge, D=16,
     lengthscale 2 with the as-printed exponent)."""

@@ -61,6 +61,11 @@ def _parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-long", action="store_true",
                     help="configs 3-4: also time the oracle's Cholesky at n=16384; config 2: also the 1-thread full pass")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "block-cyclic", "shard-predict"],
+                    help="N > 1 only. replicas (default): N independent problems, weak scaling, no data-path collective. "
+                         "block-cyclic: ONE factorisation, tile columns distributed over the ranks, panels broadcast (NCCL), strong "
+                         "scaling (SURVEY 8(f) row 2). shard-predict: replicated factor, prediction sharded by test-point tile rows "
+                         "with one all-gather of V^T, strong scaling (SURVEY 8(e)). The last two are unmeasured on hardware.")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--cusolver-ref", action="store_true")
     return ap.parse_args()
@@ -347,6 +352,81 @@ def measure_fp64_peak(gp, torch):
 LAUNCHES_PER_STEP = {"assemble": 1, "cholesky": 1, "solve": 3, "mean": 1, "full_cov": 5}   # kernels of libgp_b200.so
 
 
+def run_distributed(args):
+    """--mode block-cyclic / shard-predict: one problem on N GPUs (strong scaling), paper_2602_19683_b200/multi_gpu.py."""
+    import torch
+    import torch.distributed as dist
+    rank, local, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2602_19683_b200 import binding as gp, multi_gpu as mg, nfir
+    gp.load()
+    cfg, tile = _config(args)
+    n, m, D = cfg.n, cfg.m, cfg.D
+    h = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    X, y, Xs = nfir.make_inputs(cfg)                       # the SAME problem on every rank
+    dX, dY, dXs = (torch.from_numpy(a).cuda() for a in (X, y, Xs))
+    pipe = gp.GpPipeline(n, 0, D, tile, h, sched_width=args.width)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    times = []
+    if args.mode == "block-cyclic":
+        st = mg.MixedCholeskyRank(n, tile, pipe.KL, pipe.info, rank, world, args.width)
+        for it in range(args.warmup + args.steps):
+            pipe.assemble(dX)
+            st.reset()
+            barrier()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            if world > 1:
+                st.run()
+            else:
+                mg.run_lockstep([st])
+            b.record()
+            barrier()
+            if it >= args.warmup:
+                times.append(a.elapsed_time(b))
+        what = "Cholesky, tile columns block-cyclic over the ranks, FP64 panels broadcast, int8-emulated trailing updates"
+    else:
+        pipe.assemble(dX); pipe.cholesky(); pipe.solve(dY)   # replicated factor (not timed)
+        sp = mg.ShardedPredictor(n, m, D, tile, h, rank, world, args.width)
+        for it in range(args.warmup + args.steps):
+            barrier()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            sp.solve_local(pipe.KL, dX, dXs, pipe.alpha)
+            if world > 1:
+                sp.all_gather()
+            sp.covariance_rows(dXs)
+            b.record()
+            barrier()
+            if it >= args.warmup:
+                times.append(a.elapsed_time(b))
+        what = "full-covariance prediction given L, sharded by test-point tile rows, one all-gather of V^T"
+    ms = reduce_max_over_ranks([sum(times) / len(times)], device="cuda")[0]
+    if rank == 0:
+        flop = n ** 3 / 3.0 if args.mode == "block-cyclic" else float(n) * n * m + 2.0 * n * m * m
+        cfgd = _config_dict(cfg, tile, args.width, world)
+        cfgd["parallelism"] = f"{args.mode} over {world} GPU(s): {what}"
+        print(json.dumps({"metric": METRIC, "value": flop / (ms * 1e-3) / 1e9, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f64 panels + int8-emulated updates" if args.mode == "block-cyclic" else "f64", "data": "synthetic",
+                          "config": cfgd, "mode": args.mode, "info": int(pipe.info.item()),
+                          "note": "multi-GPU path verified by one-GPU lock-step emulation and gloo tests; unmeasured on multi-GPU hardware"}),
+              flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def run_b200(args):
     import torch
     rank, local, world = _dist_env()
@@ -604,6 +684,8 @@ def main():
         return run_sweep(args)
     if args.cusolver_ref:
         return run_cusolver_ref(args)
+    if args.mode != "replicas":
+        return run_distributed(args)
     return run_b200(args)
 
 

@@ -138,6 +138,21 @@ int gp_predict_variance(const double* dL, const double* dX, int64_t n, int D, co
                         gp_hyper h, int tile, int sched_width, double* dVar, void* dWork, size_t work_bytes,
                         void* stream);
 
+/* Prediction sharded by test-point tile rows (V and the mean are independent per block of
+ * test points, Sigma needs V of all of them once).  The two halves a multi-GPU driver needs
+ * (paper_2602_19683_b200/multi_gpu.py, ShardedPredictor: all-gather of V^T between them):
+ *   gp_predict_vt        dVt [m x n as GP_GENERAL tiles]  <-  V^T = K_{X^,X} L^-T for the m test points given (a11);
+ *                        arguments and workspace as gp_predict_full_cov.
+ *   gp_predict_cov_rows  dSigmaRows [rows x m] dense row-major  <-  K_{X^_r, X^} - V_r^T (V^T)^T  for the test points
+ *                        [row0, row0 + rows) against ALL m (a12), from the complete dVtAll [m x n, GP_GENERAL tiles] and
+ *                        dXsAll [m x D].  Full block rows are computed (no symmetry across callers); row0 % tile == 0,
+ *                        rows % tile == 0.  dWork: at least gp_cov_rows_workspace_bytes(). */
+int gp_predict_vt(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
+                  int sched_width, double* dVt, void* dWork, size_t work_bytes, void* stream);
+int gp_cov_rows_workspace_bytes(int64_t n, int64_t m, int64_t rows, int tile, size_t* bytes);
+int gp_predict_cov_rows(const double* dVtAll, const double* dXsAll, int64_t n, int64_t m, int D, int64_t row0, int64_t rows,
+                        gp_hyper h, int tile, int sched_width, double* dSigmaRows, void* dWork, size_t work_bytes, void* stream);
+
 /* SURVEY.md 8(f) row 4 (hyperparameters "are typically subject to optimization"): the
  * objective of that optimisation, *d_out (device double) <- log p(y) = -1/2 y^T alpha - sum_i log L_ii
  * - n/2 log(2 pi), from the factor of gp_cholesky_tiled and the alpha of gp_solve.  One CTA, fixed
@@ -218,6 +233,23 @@ int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes
 int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes);
 int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
                             void* stream);
+/* The steps of gp_cholesky_tiled_mixed as separate stream-ordered calls, so that a driver can interleave them with
+ * communication ("extend the library to distributed multi-GPU environments":
+ * paper_2602_19683_b200/multi_gpu.py distributes the tile columns block-cyclically and broadcasts each finished panel):
+ *   gp_mixed_begin          zero the counters, find the fixed-point scale from diag(K) (dKL must hold K's diagonal tiles);
+ *   gp_mixed_update_column  tile column J (tiles (I,J), I >= J)  -=  L(J:, k0:k1) L(J, k0:k1)^T  over the tile columns
+ *                           [k_tile0, k_tile1), k_tile1 <= J, from the digit planes (which must hold those columns);
+ *   gp_mixed_panel          FP64 POTRF tile task of (J,J) + TRSM tile tasks below it; column J must have received the
+ *                           updates of ALL tile columns < J;
+ *   gp_mixed_slice_column   digit planes of the tiles (I,J), I > J, of the FINAL factor (computed here or received).
+ * Same dWork (gp_mixed_workspace_bytes) for every call of one factorisation. */
+int gp_mixed_begin(const double* dKL, int64_t n, int tile, int* d_info, void* dWork, size_t work_bytes, void* stream);
+int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, int k_tile0, int k_tile1, void* dWork, size_t work_bytes,
+                           void* stream);
+int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                   void* stream);
+int gp_mixed_slice_column(const double* dKL, int64_t n, int tile, int J, void* dWork, size_t work_bytes, void* stream);
+
 /* Host-only replay check of the panel schedule of step J (returns the number of work items, or a negative GP_ERR_*). */
 int gp_panel_schedule_selfcheck(int64_t n, int tile, int J);
 

@@ -26,7 +26,9 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
            "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
-           "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck")
+           "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
+           "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
+           "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows")
 
 
 class gp_hyper(ctypes.Structure):
@@ -72,6 +74,9 @@ def load() -> ctypes.CDLL:
     lib.gp_predict_full_cov.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_predict_variance.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_log_marginal_likelihood.argtypes = [vp, i64, ci, vp, vp, vp, vp]
+    lib.gp_predict_vt.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
+    lib.gp_cov_rows_workspace_bytes.argtypes = [i64, i64, i64, ci, psz]
+    lib.gp_predict_cov_rows.argtypes = [vp, vp, i64, i64, ci, i64, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_workspace_bytes.argtypes = [i64, i64, ci, ci, psz, psz, psz]
     lib.gp_tiles_to_dense.argtypes = [vp, i64, i64, ci, ci, vp, vp]
     lib.gp_cholesky_task_counts.argtypes = [i64, ci, ctypes.POINTER(i64), ctypes.POINTER(i64)]
@@ -91,6 +96,10 @@ def load() -> ctypes.CDLL:
     lib.gp_mixed_workspace_bytes.argtypes = [i64, ci, psz]
     lib.gp_cholesky_tiled_mixed.argtypes = [vp, i64, ci, ci, vp, vp, sz, vp]
     lib.gp_panel_schedule_selfcheck.argtypes = [i64, ci, ci]
+    lib.gp_mixed_begin.argtypes = [vp, i64, ci, vp, vp, sz, vp]
+    lib.gp_mixed_update_column.argtypes = [vp, i64, ci, ci, ci, ci, vp, sz, vp]
+    lib.gp_mixed_panel.argtypes = [vp, i64, ci, ci, ci, vp, vp, sz, vp]
+    lib.gp_mixed_slice_column.argtypes = [vp, i64, ci, ci, vp, sz, vp]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
     lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
     lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
@@ -188,6 +197,27 @@ def gp_predict_variance(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: H
     m = Xs.shape[0]
     _check(load().gp_predict_variance(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(var),
                                       _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_variance")
+
+
+def gp_predict_vt(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int, Vt: torch.Tensor,
+                  work: torch.Tensor) -> None:
+    """Vt [m x n, GP_GENERAL tiles, flat] <- K_{X^,X} L^-T for the m test points of Xs."""
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_vt(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(Vt), _ptr(work, torch.uint8),
+                                work.numel(), _stream()), "gp_predict_vt")
+
+
+def gp_predict_cov_rows(Vt_all: torch.Tensor, Xs_all: torch.Tensor, n: int, row0: int, rows: int, h: Hyper, tile: int, sched_width: int,
+                        Sigma_rows: torch.Tensor, work: torch.Tensor) -> None:
+    """Sigma_rows [rows x m] <- K_{X^_r,X^} - V_r^T (V^T)^T for the test points [row0, row0 + rows)."""
+    m, D = Xs_all.shape
+    need = ctypes.c_size_t(0)
+    _check(load().gp_cov_rows_workspace_bytes(n, m, rows, tile, ctypes.byref(need)), "gp_cov_rows_workspace_bytes")
+    if work.numel() < need.value:
+        raise GpError(ERR["WORKSPACE"], "gp_predict_cov_rows")
+    _check(load().gp_predict_cov_rows(_ptr(Vt_all), _ptr(Xs_all), n, m, D, row0, rows, h.c(), tile, sched_width, _ptr(Sigma_rows),
+                                      _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_cov_rows")
 
 
 def gp_log_marginal_likelihood(L: torch.Tensor, n: int, tile: int, y: torch.Tensor, alpha: torch.Tensor, out: torch.Tensor) -> None:
@@ -296,6 +326,24 @@ def gp_cholesky_tiled_mixed(KL: torch.Tensor, n: int, tile: int, sched_width: in
     """gp_cholesky_tiled with the trailing updates emulated on the int8 tensor cores (opt-in)."""
     _check(load().gp_cholesky_tiled_mixed(_ptr(KL), n, tile, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8),
                                           work.numel(), _stream()), "gp_cholesky_tiled_mixed")
+
+
+def gp_mixed_begin(KL: torch.Tensor, n: int, tile: int, info: torch.Tensor, work: torch.Tensor) -> None:
+    _check(load().gp_mixed_begin(_ptr(KL), n, tile, _ptr(info, torch.int32), _ptr(work, torch.uint8), work.numel(), _stream()), "gp_mixed_begin")
+
+
+def gp_mixed_update_column(KL: torch.Tensor, n: int, tile: int, J: int, k0: int, k1: int, work: torch.Tensor) -> None:
+    _check(load().gp_mixed_update_column(_ptr(KL), n, tile, J, k0, k1, _ptr(work, torch.uint8), work.numel(), _stream()),
+           "gp_mixed_update_column")
+
+
+def gp_mixed_panel(KL: torch.Tensor, n: int, tile: int, J: int, sched_width: int, info: torch.Tensor, work: torch.Tensor) -> None:
+    _check(load().gp_mixed_panel(_ptr(KL), n, tile, J, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8), work.numel(),
+                                 _stream()), "gp_mixed_panel")
+
+
+def gp_mixed_slice_column(KL: torch.Tensor, n: int, tile: int, J: int, work: torch.Tensor) -> None:
+    _check(load().gp_mixed_slice_column(_ptr(KL), n, tile, J, _ptr(work, torch.uint8), work.numel(), _stream()), "gp_mixed_slice_column")
 
 
 def gp_panel_schedule_selfcheck(n: int, tile: int, J: int) -> int:

@@ -483,8 +483,9 @@ int gp_predict_mean(const double* dX, int64_t n, int D, const double* dAlpha, co
 
 // a9, a11, a12 (dSigma != NULL) or the variance-only variant (dSigma == NULL, dVar != NULL)
 static int run_predictor(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile,
-                         int sched_width, double* dSigma, double* dVar, void* dWork, size_t work_bytes, void* stream) {
-    if (!dL || !dX || !dXs || (!dSigma && !dVar) || !dWork) return GP_ERR_NULL;
+                         int sched_width, double* dSigma, double* dVar, void* dWork, size_t work_bytes, void* stream,
+                         double* dVtExt = nullptr) {
+    if (!dL || !dX || !dXs || (!dSigma && !dVar && !dVtExt) || !dWork) return GP_ERR_NULL;
     if (n <= 0 || m <= 0 || D <= 0 || n > (int64_t)1 << 22 || m > (int64_t)1 << 22) return GP_ERR_SIZE;
     int rc = tile_ok(n, tile);
     if (rc != GP_OK) return rc;
@@ -504,7 +505,7 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     if (rc != GP_OK) return rc;
     char* ws = (char*)dWork;
     const HyperDev hd = to_dev(h);
-    double* Vt = (double*)(ws + w.Vt);
+    double* Vt = dVtExt ? dVtExt : (double*)(ws + w.Vt);
     double* invD = (double*)(ws + w.invD);
     if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;
     // a9: K_{X^,X} (m x n, noise-free) straight into the V^T buffer; prior K_{X^,X^} straight into Sigma
@@ -546,7 +547,7 @@ static int run_predictor(const double* dL, const double* dX, int64_t n, int D, c
     if (dSigma) {
         dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
         mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
-    } else {
+    } else if (dVar) {
         // var_a = k(x^_a, x^_a) - sum_i V_ia^2 with k(x,x) = v (noise-free prior, reading A2): one warp per test point
         posterior_var_kernel<<<(unsigned)((m + 7) / 8), 256, 0, st>>>(Vt, m, n, tile, hd.vertical, dVar);
     }
@@ -563,6 +564,93 @@ int gp_predict_variance(const double* dL, const double* dX, int64_t n, int D, co
                         int sched_width, double* dVar, void* dWork, size_t work_bytes, void* stream) {
     if (!dVar) return GP_ERR_NULL;
     return run_predictor(dL, dX, n, D, dXs, m, h, tile, sched_width, nullptr, dVar, dWork, work_bytes, stream);
+}
+
+int gp_predict_vt(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile, int sched_width,
+                  double* dVt, void* dWork, size_t work_bytes, void* stream) {
+    if (!dVt) return GP_ERR_NULL;
+    return run_predictor(dL, dX, n, D, dXs, m, h, tile, sched_width, nullptr, nullptr, dWork, work_bytes, stream, dVt);
+}
+
+int gp_cov_rows_workspace_bytes(int64_t n, int64_t m, int64_t rows, int tile, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    if (n <= 0 || m <= 0 || rows <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc == GP_OK) rc = tile_ok(m, tile);
+    if (rc == GP_OK) rc = tile_ok(rows, tile);
+    if (rc != GP_OK) return rc;
+    const int b = pick_block(tile, n);
+    const size_t NBm = (size_t)(m / b);
+    *bytes = kHdrBytes + align_up(NBm * NBm * sizeof(int), 256) + align_up((size_t)(rows / b) * NBm * sizeof(Item), 256) + 256;
+    return GP_OK;
+}
+
+int gp_predict_cov_rows(const double* dVtAll, const double* dXsAll, int64_t n, int64_t m, int D, int64_t row0, int64_t rows, gp_hyper h,
+                        int tile, int sched_width, double* dSigmaRows, void* dWork, size_t work_bytes, void* stream) {
+    if (!dVtAll || !dXsAll || !dSigmaRows || !dWork) return GP_ERR_NULL;
+    if (n <= 0 || m <= 0 || D <= 0 || rows <= 0 || row0 < 0 || row0 + rows > m || n > (int64_t)1 << 22 || m > (int64_t)1 << 22) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc == GP_OK) rc = tile_ok(m, tile);
+    if (rc == GP_OK) rc = tile_ok(rows, tile);
+    if (rc != GP_OK) return rc;
+    if (row0 % tile != 0) return GP_ERR_TILE;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    const int b = pick_block(tile, n);
+    if (n / b > 65535 || m / b > 65535) return GP_ERR_SIZE;
+    size_t need = 0;
+    gp_cov_rows_workspace_bytes(n, m, rows, tile, &need);
+    if (work_bytes < need) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int NB = (int)(n / b), NBm = (int)(m / b), nrows = (int)(rows / b), gr0 = (int)(row0 / b);
+    char* ws = (char*)dWork;
+    const size_t off_ver = kHdrBytes, off_items = off_ver + align_up((size_t)NBm * NBm * sizeof(int), 256);
+    if (cudaMemsetAsync(ws, 0, off_items, st) != cudaSuccess) return GP_ERR_CUDA;
+    const HyperDev hd = to_dev(h);
+    {   // the prior K_{X^_r, X^} straight into the output rows
+        const int64_t rb = (rows + kAsmBlk - 1) / kAsmBlk, cb = (m + kAsmBlk - 1) / kAsmBlk;
+        if (rb * cb > 2147483647LL) return GP_ERR_SIZE;
+        const size_t smem = 2 * (size_t)kAsmMaxD * kAsmBlk * sizeof(double);
+        assemble_dense_kernel<<<(unsigned)(rb * cb), 256, smem, st>>>(dXsAll + row0 * D, rows, dXsAll, m, D, hd, dSigmaRows, m);
+        if (cudaGetLastError() != cudaSuccess) return GP_ERR_CUDA;
+    }
+    Item* items = (Item*)(ws + off_items);
+    cov_row_items_kernel<<<(nrows * NBm + 255) / 256, 256, 0, st>>>((uint4*)items, nrows, gr0, NBm, NB, (unsigned)OP_UPD_S);
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = const_cast<double*>(dVtAll);        // no item touches L: the pointer only has to be mappable
+    p.Vt = const_cast<double*>(dVtAll);
+    p.S = dSigmaRows;
+    p.invD = (double*)ws;
+    p.verV = (int*)(ws + off_ver);
+    p.verS = (int*)(ws + off_ver);
+    p.items = items;
+    p.nitems = nrows * NBm;
+    p.ticket = (unsigned int*)ws;
+    p.stats = (unsigned long long*)(ws + kStatsOff);
+    p.t = tile;
+    p.nbt = tile / b;
+    p.snbt = NB;                               // one version per item: the whole contraction range is one "column"
+    p.NB = NB;
+    p.NBm = NBm;
+    p.Mt = (int)(n / tile);
+    p.m = m;
+    p.s_row0 = gr0;
+    p.L_final = 1;
+    p.no_deps = 1;
+    // the L map is built over [Mt (Mt + 1) / 2 * t, t]: keep it inside the V^T buffer, which has m / t * Mt * t rows
+    {
+        ExecMaps mp;
+        int rc2 = make_map(&mp.V, dVtAll, (uint64_t)(m / tile) * (uint64_t)p.Mt * (uint64_t)tile, (uint64_t)tile, b);
+        if (rc2 != GP_OK) return rc2;
+        mp.L = mp.V;
+        mp.D = mp.V;
+        switch (b) {
+            case 128: rc = launch_exec<128>(p, mp, workers_for(sched_width), st); break;
+            case 64: rc = launch_exec<64>(p, mp, workers_for(sched_width), st); break;
+            default: rc = launch_exec<32>(p, mp, workers_for(sched_width), st); break;
+        }
+    }
+    return rc;
 }
 
 int gp_log_marginal_likelihood(const double* dL, int64_t n, int tile, const double* dY, const double* dAlpha, double* d_out,
@@ -857,46 +945,70 @@ extern "C" int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes) {
     return GP_OK;
 }
 
-extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
-                                       void* stream) {
-    if (!dKL || !d_info || !dWork) return GP_ERR_NULL;
-    int rc = mixed_ok(n, tile);
+// The four steps of the mixed factorisation.  gp_cholesky_tiled_mixed runs them in a loop; a multi-GPU driver
+// (paper_2602_19683_b200/multi_gpu.py, block-cyclic tile columns) interleaves them with panel broadcasts.
+namespace {
+struct MixedCtx {
+    MixedWs w;
+    char* ws;
+    int M, nbt, NB;
+    cudaStream_t st;
+};
+int mixed_ctx(int64_t n, int tile, void* dWork, size_t work_bytes, void* stream, MixedCtx* c) {
+    if (!dWork) return GP_ERR_NULL;
+    const int rc = mixed_ok(n, tile);
     if (rc != GP_OK) return rc;
-    const MixedWs w = mixed_ws(n);
-    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
-    cudaStream_t st = (cudaStream_t)stream;
-    constexpr int b = 128;
-    const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b);
-    const int workers = workers_for(sched_width);
-    // the panel schedules of all M steps (built and uploaded on first use, like the other schedules)
-    std::vector<CachedSchedule> panels(M);
-    {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
-        std::lock_guard<std::mutex> lk(g_mu);
-        for (int J = 0; J < M; ++J) {
-            auto key = std::make_tuple(dev, 16 + J, M, 0, nbt, b);
-            auto it = g_cache.find(key);
-            if (it != g_cache.end()) { panels[J] = it->second; continue; }
-            std::vector<SchedItem> items;
-            build_panel_schedule(M, nbt, J, sm_count(), items, b);
-            CachedSchedule cs;
-            cs.nitems = (int)items.size();
-            if (cudaMalloc(&cs.d_items, items.size() * sizeof(Item) + 16) != cudaSuccess) return GP_ERR_CUDA;
-            if (cudaMemcpy(cs.d_items, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice) != cudaSuccess) {
-                cudaFree(cs.d_items);
-                return GP_ERR_CUDA;
-            }
-            g_cache[key] = cs;
-            panels[J] = cs;
-        }
+    c->w = mixed_ws(n);
+    if (work_bytes < c->w.total) return GP_ERR_WORKSPACE;
+    c->ws = (char*)dWork;
+    c->M = (int)(n / tile);
+    c->nbt = tile / 128;
+    c->NB = (int)(n / 128);
+    c->st = (cudaStream_t)stream;
+    return GP_OK;
+}
+int get_panel_schedule(int M, int nbt, int J, CachedSchedule* out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto key = std::make_tuple(dev, 16 + J, M, 0, nbt, 128);
+    auto it = g_cache.find(key);
+    if (it != g_cache.end()) { *out = it->second; return GP_OK; }
+    std::vector<SchedItem> items;
+    build_panel_schedule(M, nbt, J, sm_count(), items, 128);
+    CachedSchedule cs;
+    cs.nitems = (int)items.size();
+    if (cudaMalloc(&cs.d_items, items.size() * sizeof(Item) + 16) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemcpy(cs.d_items, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaFree(cs.d_items);
+        return GP_ERR_CUDA;
     }
-    char* ws = (char*)dWork;
-    double* d_scale = (double*)(ws + w.scale);
-    int8_t* planes = (int8_t*)(ws + w.planes);
-    if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;           // tickets, statistics, version counters
-    if (cudaMemsetAsync(d_info, 0, sizeof(int), st) != cudaSuccess) return GP_ERR_CUDA;
-    oz::factor_scale_kernel<<<1, 1024, 0, st>>>(dKL, n, tile, d_scale);
+    g_cache[key] = cs;
+    *out = cs;
+    return GP_OK;
+}
+}  // namespace
+
+extern "C" int gp_mixed_begin(const double* dKL, int64_t n, int tile, int* d_info, void* dWork, size_t work_bytes, void* stream) {
+    if (!dKL || !d_info) return GP_ERR_NULL;
+    MixedCtx c;
+    const int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
+    if (rc != GP_OK) return rc;
+    if (cudaMemsetAsync(c.ws, 0, c.w.invD, c.st) != cudaSuccess) return GP_ERR_CUDA;          // tickets, statistics, version counters
+    if (cudaMemsetAsync(d_info, 0, sizeof(int), c.st) != cudaSuccess) return GP_ERR_CUDA;
+    oz::factor_scale_kernel<<<1, 1024, 0, c.st>>>(dKL, n, tile, (double*)(c.ws + c.w.scale));
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, int k_tile0, int k_tile1, void* dWork, size_t work_bytes,
+                                      void* stream) {
+    if (!dKL) return GP_ERR_NULL;
+    MixedCtx c;
+    int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
+    if (rc != GP_OK) return rc;
+    if (J < 0 || J >= c.M || k_tile0 < 0 || k_tile1 > J || k_tile0 > k_tile1) return GP_ERR_SIZE;
+    if (k_tile0 == k_tile1) return GP_OK;
+    int8_t* planes = (int8_t*)(c.ws + c.w.planes);
     // one tensor map over the dense digit planes [8][n][n] for both operands (boxes of 128 and of 64 rows)
     CUtensorMap mapA, mapB;
     if ((rc = make_plane_map(&mapA, planes, (uint64_t)n, (uint64_t)n, oz::kTileM)) != GP_OK) return rc;
@@ -905,51 +1017,82 @@ extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sch
         return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
     });
     if (rc != GP_OK) return rc;
+    oz::OzParams q;
+    memset(&q, 0, sizeof(q));
+    q.C = dKL;
+    q.tiles_m = (c.M - J) * (tile / oz::kTileM);
+    q.tiles_n = tile / oz::kTileN;
+    q.kchunks = (int)((int64_t)(k_tile1 - k_tile0) * tile / oz::kChunk);
+    q.kc0 = (int)((int64_t)k_tile0 * tile / oz::kChunk);
+    q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+    q.scale = (const double*)(c.ws + c.w.scale);
+    q.tiled = 1;
+    q.t = tile;
+    q.J = J;
+    q.row0 = J * tile;
+    const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
+    oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, c.st>>>(q, mapA, mapB);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                              void* stream) {
+    if (!dKL || !d_info) return GP_ERR_NULL;
+    MixedCtx c;
+    int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
+    if (rc != GP_OK) return rc;
+    if (J < 0 || J >= c.M) return GP_ERR_SIZE;
+    CachedSchedule cs;
+    if ((rc = get_panel_schedule(c.M, c.nbt, J, &cs)) != GP_OK) return rc;
     ExecParams p;
     memset(&p, 0, sizeof(p));
     p.L = dKL;
-    p.invD = (double*)(ws + w.invD);
-    p.verL = (int*)(ws + w.verL);
-    p.stats = (unsigned long long*)(ws + kStatsOff);
+    p.invD = (double*)(c.ws + c.w.invD);
+    p.verL = (int*)(c.ws + c.w.verL);
+    p.stats = (unsigned long long*)(c.ws + kStatsOff);
     p.d_info = d_info;
     p.t = tile;
-    p.nbt = nbt;
-    p.snbt = nbt;
-    p.NB = NB;
-    p.Mt = M;
+    p.nbt = c.nbt;
+    p.snbt = c.nbt;
+    p.NB = c.NB;
+    p.Mt = c.M;
+    p.items = cs.d_items;
+    p.nitems = cs.nitems;
+    p.ticket = (unsigned int*)(c.ws + c.w.ticket) + J;
     ExecMaps mp;
-    if ((rc = make_exec_maps(&mp, p, b, 0)) != GP_OK) return rc;
-    for (int J = 0; J < M; ++J) {
-        if (J > 0) {
-            // left-looking: tile column J -= L(J:, 0:J) L(J, 0:J)^T, one emulated contraction of depth J * tile
-            oz::OzParams q;
-            memset(&q, 0, sizeof(q));
-            q.C = dKL;
-            q.tiles_m = (M - J) * (tile / oz::kTileM);
-            q.tiles_n = tile / oz::kTileN;
-            q.kchunks = (int)((int64_t)J * tile / oz::kChunk);
-            q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
-            q.scale = d_scale;
-            q.tiled = 1;
-            q.t = tile;
-            q.J = J;
-            q.row0 = J * tile;
-            const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
-            oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
-            oz::set_column_versions_kernel<<<(NB * nbt + 255) / 256, 256, 0, st>>>(p.verL, NB, nbt, J, kConsumerWarps);
-        }
-        p.items = panels[J].d_items;
-        p.nitems = panels[J].nitems;
-        p.ticket = (unsigned int*)(ws + w.ticket) + J;
-        rc = launch_exec<128>(p, mp, workers, st);
-        if (rc != GP_OK) return rc;
-        if (J + 1 < M) {
-            const int64_t total = (n - (int64_t)(J + 1) * tile) * (tile / 4);
-            const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
-            oz::slice_tile_column_kernel<<<grid, 256, 0, st>>>(dKL, n, tile, J, d_scale, planes);
-        }
-    }
+    if ((rc = make_exec_maps(&mp, p, 128, 0)) != GP_OK) return rc;
+    // the J trailing updates of this column were applied by the emulated contraction, outside the executor's counters
+    if (cudaMemsetAsync(p.ticket, 0, sizeof(unsigned int), c.st) != cudaSuccess) return GP_ERR_CUDA;
+    oz::set_column_versions_kernel<<<(c.NB * c.nbt + 255) / 256, 256, 0, c.st>>>(p.verL, c.NB, c.nbt, J, kConsumerWarps);
+    return launch_exec<128>(p, mp, workers_for(sched_width), c.st);
+}
+
+extern "C" int gp_mixed_slice_column(const double* dKL, int64_t n, int tile, int J, void* dWork, size_t work_bytes, void* stream) {
+    if (!dKL) return GP_ERR_NULL;
+    MixedCtx c;
+    const int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
+    if (rc != GP_OK) return rc;
+    if (J < 0 || J >= c.M) return GP_ERR_SIZE;
+    if (J + 1 == c.M) return GP_OK;                          // the last column has no tile below its diagonal tile
+    const int64_t total = (n - (int64_t)(J + 1) * tile) * (tile / 4);
+    const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
+    oz::slice_tile_column_kernel<<<grid, 256, 0, c.st>>>(dKL, n, tile, J, (const double*)(c.ws + c.w.scale), (int8_t*)(c.ws + c.w.planes));
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                                       void* stream) {
+    int rc = gp_mixed_begin(dKL, n, tile, d_info, dWork, work_bytes, stream);
+    if (rc != GP_OK) return rc;
+    const int M = (int)(n / tile);
+    for (int J = 0; J < M; ++J) {
+        // left-looking: tile column J -= L(J:, 0:J) L(J, 0:J)^T in one emulated contraction of depth J * tile, then its
+        // FP64 panel step, then its digit planes
+        if ((rc = gp_mixed_update_column(dKL, n, tile, J, 0, J, dWork, work_bytes, stream)) != GP_OK) return rc;
+        if ((rc = gp_mixed_panel(dKL, n, tile, J, sched_width, d_info, dWork, work_bytes, stream)) != GP_OK) return rc;
+        if ((rc = gp_mixed_slice_column(dKL, n, tile, J, dWork, work_bytes, stream)) != GP_OK) return rc;
+    }
+    return GP_OK;
 }
 
 extern "C" int gp_panel_schedule_selfcheck(int64_t n, int tile, int J) {

@@ -72,7 +72,8 @@ struct ExecParams {
     int NB;                // n / b
     int NBm;               // m / b
     int Mt;                // n / t (tiles per row of V^T)
-    int64_t m;             // rows of Sigma (leading dimension)
+    int64_t m;             // leading dimension of Sigma
+    int s_row0;            // block row of V^T that row 0 of S corresponds to (0 except for the sharded block rows of Sigma)
     int L_final;           // 1: L is an input that is final everywhere (predictor), no waits on it
     int no_deps;           // 1: skip every dependency wait (contraction microbenchmark only)
     unsigned long long* stats;   // 8 per worker CTA, see gp_exec_stats in include/gp_b200.h
@@ -140,7 +141,7 @@ struct Producer {
         return p.Vt + ((size_t)I * p.Mt + J) * (size_t)p.t * p.t + (size_t)(gr % p.nbt) * BLK * p.t +
                (size_t)(gc % p.nbt) * BLK;
     }
-    __device__ __forceinline__ double* blkS(int gr, int gc) const { return p.S + (size_t)gr * BLK * p.m + (size_t)gc * BLK; }
+    __device__ __forceinline__ double* blkS(int gr, int gc) const { return p.S + (size_t)(gr - p.s_row0) * BLK * p.m + (size_t)gc * BLK; }
     // TMA coordinates {inner element, row} of block (gr, gc) in the [tiles*t, t] view of L / V^T
     __device__ __forceinline__ int2 crdL(int gr, int gc) const {
         const int I = gr / p.nbt, J = gc / p.nbt;

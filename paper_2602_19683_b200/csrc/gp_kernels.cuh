@@ -135,6 +135,63 @@ __global__ void __launch_bounds__(256) assemble_tiles_kernel(const double* __res
     }
 }
 
+// Dense rectangular variant: out [na x nb] row-major with leading dimension ld, out(i, j) = k(A_i, B_j), never any noise
+// (the prior K_{X^_r, X^} of a block of test points against all of them, for the sharded covariance rows).
+__global__ void __launch_bounds__(256) assemble_dense_kernel(const double* __restrict__ A, int64_t na, const double* __restrict__ B,
+                                                             int64_t nb, int D, HyperDev h, double* __restrict__ out, int64_t ld) {
+    extern __shared__ __align__(16) double sm[];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int64_t cb = (nb + kAsmBlk - 1) / kAsmBlk;
+    const int64_t gi0 = (int64_t)(blockIdx.x / cb) * kAsmBlk, gj0 = (int64_t)(blockIdx.x % cb) * kAsmBlk;
+    const int nrow = (int)min((int64_t)kAsmBlk, na - gi0), ncol = (int)min((int64_t)kAsmBlk, nb - gj0);
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    double* sA = sm;
+    double* sB = sm + kAsmMaxD * kAsmBlk;
+    for (int d0 = 0; d0 < D; d0 += kAsmMaxD) {
+        const int dc = min(kAsmMaxD, D - d0);
+        __syncthreads();
+        for (int idx = tid; idx < kAsmBlk * dc; idx += 256) {
+            const int r = idx / dc, d = idx % dc;
+            sA[d * kAsmBlk + r] = (r < nrow) ? A[(gi0 + r) * D + d0 + d] : 0.0;
+            sB[d * kAsmBlk + r] = (r < ncol) ? B[(gj0 + r) * D + d0 + d] : 0.0;
+        }
+        __syncthreads();
+        for (int d = 0; d < dc; ++d) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = sA[d * kAsmBlk + ty + 16 * i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = sB[d * kAsmBlk + 4 * tx + j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const double diff = a[i] - b[j];
+                    acc[i][j] = fma(diff, diff, acc[i][j]);
+                }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int r = ty + 16 * i;
+        if (r >= nrow) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (4 * tx + j < ncol) out[(gi0 + r) * ld + gj0 + 4 * tx + j] = se_kernel(acc[i][j], h);
+    }
+}
+
+// work items of the sharded covariance rows: block row gr0 + i of V^T against every block row gc, the whole contraction
+// range in one item (no item depends on another)
+__global__ void cov_row_items_kernel(uint4* __restrict__ items, int rows, int gr0, int NBm, int NB, unsigned op) {
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < rows * NBm; idx += gridDim.x * blockDim.x)
+        items[idx] = make_uint4(op, (unsigned)(gr0 + idx / NBm), (unsigned)(idx % NBm), (unsigned)NB << 16);
+}
+
 // tiles -> dense (inspection helper)
 __global__ void tiles_to_dense_kernel(const double* __restrict__ tiles, int64_t n, int64_t nb, int tile, int lower_packed,
                                       double* __restrict__ dense) {

@@ -199,6 +199,7 @@ struct OzParams {
     // tile row J down; operand rows and the k extent are taken from dense digit planes of the whole matrix
     int tiled, t, J;
     int row0;             // first operand row of A and of B in the planes (J * t)
+    int kc0;              // first k-chunk (the contraction covers the chunks [kc0, kc0 + kchunks))
 };
 
 // tile (tm, tn) -> is it wanted, and where does row `r` (0..127) of it live
@@ -260,8 +261,8 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
                     mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
                     char* dst = base + (size_t)stage * kStageBytesOz;
                     mbar_arrive_expect_tx(&full[stage], (uint32_t)kStageBytesOz);
-                    tma_load_3d(dst, &mapA, kc * kChunk, p.row0 + tm * kTileM, 0, &full[stage]);
-                    tma_load_3d(dst + kABytes, &mapB, kc * kChunk, p.row0 + tn * kTileN, 0, &full[stage]);
+                    tma_load_3d(dst, &mapA, (p.kc0 + kc) * kChunk, p.row0 + tm * kTileM, 0, &full[stage]);
+                    tma_load_3d(dst + kABytes, &mapB, (p.kc0 + kc) * kChunk, p.row0 + tn * kTileN, 0, &full[stage]);
                     if (++stage == kStagesOz) { stage = 0; phase ^= 1; }
                 }
             }

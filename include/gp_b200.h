@@ -215,6 +215,11 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
  * Both calls are stream-ordered.  This is a measured building block (bench.py reports its FP64-equivalent rate
  * beside the DMMA contraction); gp_cholesky_tiled does not use it. */
 int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes);
+/* Output-tile shape of the emulated contraction: 64 (= 0 = auto: 128 x 64 output tile, all eight level sums resident in
+ * tensor memory, one pass over k) or 128 (128 x 128 output tile, the levels in two passes of four; needs a column count
+ * that is a multiple of 128).  Both were measured at the same 2.3-2.45 int8 POPS (they move the same bytes from L2 to
+ * shared memory per product, which is what bounds them); measurement support. */
+int gp_set_ozaki_tile_n(int n);
 int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double scale, int8_t* dPlanes, int* d_overflow,
                    void* stream);
 int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,

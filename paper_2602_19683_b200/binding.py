@@ -28,7 +28,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
-           "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows")
+           "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n")
 
 
 class gp_hyper(ctypes.Structure):
@@ -101,6 +101,7 @@ def load() -> ctypes.CDLL:
     lib.gp_mixed_panel.argtypes = [vp, i64, ci, ci, ci, vp, vp, sz, vp]
     lib.gp_mixed_slice_column.argtypes = [vp, i64, ci, ci, vp, sz, vp]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
+    lib.gp_set_ozaki_tile_n.argtypes = [ci]
     lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
     lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
     lib.gp_block_size_for.argtypes = [i64, ci]
@@ -348,6 +349,10 @@ def gp_mixed_slice_column(KL: torch.Tensor, n: int, tile: int, J: int, work: tor
 
 def gp_panel_schedule_selfcheck(n: int, tile: int, J: int) -> int:
     return int(load().gp_panel_schedule_selfcheck(n, tile, J))
+
+
+def gp_set_ozaki_tile_n(n: int) -> None:
+    _check(load().gp_set_ozaki_tile_n(int(n)), "gp_set_ozaki_tile_n")
 
 
 def gp_ozaki_slice(X: torch.Tensor, scale: float) -> torch.Tensor:

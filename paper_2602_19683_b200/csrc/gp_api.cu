@@ -849,12 +849,12 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
 // ---- split-operand (Ozaki) contraction on the int8 tensor cores -------------------------
 namespace {
 // planes [S][rows][k] (int8) viewed through boxes of {32 bytes of k, box_rows rows, all S planes}, 32-byte swizzle
-int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64_t k, uint32_t box_rows) {
+int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64_t k, uint32_t box_rows, uint32_t box_planes = oz::kPlanes) {
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return GP_ERR_CUDA;
     const cuuint64_t dims[3] = {(cuuint64_t)k, (cuuint64_t)rows, (cuuint64_t)oz::kPlanes};
     const cuuint64_t strides[2] = {(cuuint64_t)k, (cuuint64_t)(rows * k)};
-    const cuuint32_t box[3] = {(cuuint32_t)oz::kChunk, box_rows, (cuuint32_t)oz::kPlanes};
+    const cuuint32_t box[3] = {(cuuint32_t)oz::kChunk, box_rows, box_planes};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<int8_t*>(planes), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -862,6 +862,47 @@ int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64
     return r == CUDA_SUCCESS ? GP_OK : GP_ERR_CUDA;
 }
 }  // namespace
+
+namespace {
+std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (= 64: see gp_ozaki.cuh), 64, 128: gp_set_ozaki_tile_n (measurement support)
+
+// launches the emulated contraction described by q (tiles_n counted in 64-column units on entry) with the chosen tile shape
+int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const int8_t* planesB, uint64_t rowsB, uint64_t kdim, int64_t ncols,
+                 cudaStream_t st) {
+    const int want = g_ozaki_tile_n.load(std::memory_order_relaxed);
+    const bool wide = want == 128 && ncols % oz::kTileN2 == 0;
+    CUtensorMap mapA, mapB;
+    int rc;
+    if (wide) {
+        if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM, 4)) != GP_OK) return rc;
+        if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN2, 4)) != GP_OK) return rc;
+        rc = configure_once(1024u, [] {
+            return cudaFuncSetAttribute(oz::ozaki_contract_kernel2, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz2) == cudaSuccess;
+        });
+        if (rc != GP_OK) return rc;
+        q.tiles_n = (int)(ncols / oz::kTileN2);
+        const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
+        oz::ozaki_contract_kernel2<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz2, st>>>(q, mapA, mapB);
+    } else {
+        if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM)) != GP_OK) return rc;
+        if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN)) != GP_OK) return rc;
+        rc = configure_once(512u, [] {
+            return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
+        });
+        if (rc != GP_OK) return rc;
+        q.tiles_n = (int)(ncols / oz::kTileN);
+        const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
+        oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
+    }
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+}  // namespace
+
+extern "C" int gp_set_ozaki_tile_n(int n) {
+    if (n != 0 && n != 64 && n != 128) return GP_ERR_SIZE;
+    g_ozaki_tile_n.store(n, std::memory_order_relaxed);
+    return GP_OK;
+}
 
 extern "C" int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes) {
     if (!bytes) return GP_ERR_NULL;
@@ -890,26 +931,14 @@ extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_
     if (ma <= 0 || nb <= 0 || k <= 0 || ma % oz::kTileM != 0 || nb % oz::kTileN != 0 || k % oz::kChunk != 0 || k > 65536 || ldc < nb || ldc % 2 != 0)
         return GP_ERR_SIZE;
     if (!(scaleA > 0.0) || !(scaleB > 0.0) || !std::isfinite(scaleA * scaleB)) return GP_ERR_HYPER;
-    CUtensorMap mapA, mapB;
-    int rc = make_plane_map(&mapA, dAplanes, (uint64_t)ma, (uint64_t)k, oz::kTileM);
-    if (rc != GP_OK) return rc;
-    if ((rc = make_plane_map(&mapB, dBplanes, (uint64_t)nb, (uint64_t)k, oz::kTileN)) != GP_OK) return rc;
-    rc = configure_once(512u, [] {
-        return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
-    });
-    if (rc != GP_OK) return rc;
     oz::OzParams p;
     memset(&p, 0, sizeof(p));
     p.C = dC;
     p.ldc = ldc;
     p.tiles_m = (int)(ma / oz::kTileM);
-    p.tiles_n = (int)(nb / oz::kTileN);
     p.kchunks = (int)(k / oz::kChunk);
     p.w_last = scaleA * scaleB * std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
-    const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
-    const int grid = (int)std::min<int64_t>(tiles, sm_count());
-    oz::ozaki_contract_kernel<<<grid, oz::kThreadsOz, oz::kSmemOz, (cudaStream_t)stream>>>(p, mapA, mapB);
-    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+    return launch_ozaki(p, dAplanes, (uint64_t)ma, dBplanes, (uint64_t)nb, (uint64_t)k, nb, (cudaStream_t)stream);
 }
 
 // ---- gp_cholesky_tiled_mixed: FP64 panels + emulated trailing updates ------------------------
@@ -1009,19 +1038,10 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     if (J < 0 || J >= c.M || k_tile0 < 0 || k_tile1 > J || k_tile0 > k_tile1) return GP_ERR_SIZE;
     if (k_tile0 == k_tile1) return GP_OK;
     int8_t* planes = (int8_t*)(c.ws + c.w.planes);
-    // one tensor map over the dense digit planes [8][n][n] for both operands (boxes of 128 and of 64 rows)
-    CUtensorMap mapA, mapB;
-    if ((rc = make_plane_map(&mapA, planes, (uint64_t)n, (uint64_t)n, oz::kTileM)) != GP_OK) return rc;
-    if ((rc = make_plane_map(&mapB, planes, (uint64_t)n, (uint64_t)n, oz::kTileN)) != GP_OK) return rc;
-    rc = configure_once(512u, [] {
-        return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
-    });
-    if (rc != GP_OK) return rc;
     oz::OzParams q;
     memset(&q, 0, sizeof(q));
     q.C = dKL;
     q.tiles_m = (c.M - J) * (tile / oz::kTileM);
-    q.tiles_n = tile / oz::kTileN;
     q.kchunks = (int)((int64_t)(k_tile1 - k_tile0) * tile / oz::kChunk);
     q.kc0 = (int)((int64_t)k_tile0 * tile / oz::kChunk);
     q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
@@ -1030,9 +1050,8 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     q.t = tile;
     q.J = J;
     q.row0 = J * tile;
-    const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
-    oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, c.st>>>(q, mapA, mapB);
-    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+    // both operands come from the dense digit planes [8][n][n] of the whole matrix
+    return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, c.st);
 }
 
 extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,

@@ -30,10 +30,17 @@
 // on three matrices: L (lower-packed tiles), V^T (general tiles) and Sigma (dense).
 //
 // Deadlock freedom: the item list is a topological order of the DAG and tickets are handed out
-// in list order.  A CTA holds at most two tickets (the one its consumers run and the one its
-// producer prepares); the unfinished item with the lowest ticket is therefore always the one some
-// CTA's consumers are running (an earlier ticket of the same CTA would be unfinished and lower),
-// all its dependencies are finished, so it completes.
+// in list order.  A CTA holds up to three tickets at once (the item its consumers run, a short item
+// that is already completely streamed into the ring behind it, and the one its producer is polling
+// for), but it works through them IN ticket order, and a producer only polls for item k after it
+// has handed over every earlier ticket of its CTA.  So consider the unfinished item with the lowest
+// ticket: every dependency of it has a lower ticket and is therefore finished, its producer's poll
+// succeeds, and every earlier ticket of the same CTA is finished, so its consumers reach it: it
+// completes.  By induction every item completes.
+// Versions: a merged update raises its block's counter by several versions in steps that are not
+// ordered among the eight consumer warps, so the versions strictly INSIDE such a write are never a
+// state in which the block is complete; no item may wait for one of them, and
+// validate_schedule (gp_schedule.cpp) rejects a schedule in which one does.
 #pragma once
 #include "gp_diag.cuh"
 #include "gp_gemm.cuh"

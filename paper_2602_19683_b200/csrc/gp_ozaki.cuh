@@ -208,20 +208,21 @@ struct OzTile {
     double* c;            // address of element (row 0 of the tile, column 0 of the tile)
     int64_t ld;
 };
+template <int TN = kTileN>
 __device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
     OzTile o;
     if (!p.tiled) {
         o.wanted = true;
         o.ld = p.ldc;
-        o.c = p.C + (size_t)tm * kTileM * p.ldc + (size_t)tn * kTileN;
+        o.c = p.C + (size_t)tm * kTileM * p.ldc + (size_t)tn * TN;
         return o;
     }
     const int bpt = p.t / kTileM;                       // 128-row blocks per tile edge
     const int I = p.J + tm / bpt, rblk = tm % bpt;
-    // on the diagonal tile only the lower part is data: skip 128 x 64 pieces that lie wholly above the diagonal
-    o.wanted = !(I == p.J && tn * kTileN >= (rblk + 1) * kTileM);
+    // on the diagonal tile only the lower part is data: skip 128 x TN pieces that lie wholly above the diagonal
+    o.wanted = !(I == p.J && tn * TN >= (rblk + 1) * kTileM);
     o.ld = p.t;
-    o.c = p.C + ((size_t)I * (I + 1) / 2 + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * kTileN;
+    o.c = p.C + ((size_t)I * (I + 1) / 2 + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * TN;
     return o;
 }
 
@@ -334,6 +335,164 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
             __syncwarp();
             if (lane == 0) mbar_arrive(tmem_empty);
             tphase ^= 1;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+
+// ---- second shape: 128 x 128 output tile, the eight levels in TWO passes of four ---------------------------------------
+// The 128 x 64 kernel above keeps all eight level sums in tensor memory, so every operand byte is fetched once -- but each
+// of its MMAs (128 x 64 x 32) makes the tensor core read 4 KB of A and 2 KB of B from shared memory for 32 cycles of
+// work: 192 B/cycle against a shared-memory port of 128 B/cycle.  With N = 128 an MMA reads 4 + 4 KB for 64 cycles
+// (128 B/cycle), and tensor memory holds four level sums of 128 columns: the levels are done in two passes over k
+// (levels 0-3 need the planes 0-3 only: 10 products per chunk; levels 4-7 need all planes: 26), which costs exactly the
+// L2 traffic the 128 x 64 kernel spends on loading A once per column half.
+// MEASURED (8192 x 8192 x k, FP64-equivalent TFLOP/s): k = 1024 / 4096 / 16384: 128 x 64: 59.7 / 63.4 / 64.7;
+// 128 x 128: 51.8 / 68.1 / 62.7.  The two shapes end at the same 2.3-2.45 int8 POPS although their shared-memory
+// demand differs by a third: what they share is the 96 KB per 128 x 128 x 32 product that travel from L2 to shared
+// memory (5.9 TB/s over the chip at that rate), so that, not the operand read of the tensor core, is the bound.  The
+// way past it is a larger output tile per operand byte (a CTA pair with cta_group::2 / TMA multicast); not built.
+// The 128 x 64 shape is the default (no second pass, so no drain bubble at short k).
+constexpr int kTileN2 = 128;
+constexpr int kSlotBytes2 = 2 * kPlanes * kTileM * kChunk;          // 64 KB: 8 planes of A + 8 planes of B, one k-chunk
+constexpr int kStages2 = 3;
+constexpr int kSmemOz2 = kStages2 * kSlotBytes2 + 1024 + 256;
+constexpr uint32_t kIdescI8N128 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTileN2 >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+
+// map4: boxes of {32 bytes of k, 128 rows, 4 planes} (the same box serves A and B)
+__global__ void __launch_bounds__(kThreadsOz, 1)
+ozaki_contract_kernel2(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
+    extern __shared__ char smem_raw[];
+    char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + kStages2 * kSlotBytes2);
+    uint64_t* empty = full + kStages2;
+    uint64_t* tmem_full = empty + kStages2;
+    uint64_t* tmem_empty = tmem_full + 1;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 1);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages2; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        mbar_init(tmem_full, 1);
+        mbar_init(tmem_empty, 4);
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+    const int ntiles = p.tiles_m * p.tiles_n;
+    constexpr int kPlaneBytes = kTileM * kChunk;                    // 4 KB
+    constexpr int kHalf = 4 * kPlaneBytes;                          // one TMA box: 4 planes
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            tma_prefetch_desc(&mapA);
+            tma_prefetch_desc(&mapB);
+            int stage = 0, phase = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const int tm = tile / p.tiles_n, tn = tile % p.tiles_n;
+                if (!oz_tile<kTileN2>(p, tm, tn).wanted) continue;
+                for (int pass = 0; pass < 2; ++pass)
+                    for (int kc = 0; kc < p.kchunks; ++kc) {
+                        mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
+                        char* dst = base + (size_t)stage * kSlotBytes2;
+                        const int k = (p.kc0 + kc) * kChunk, ra = p.row0 + tm * kTileM, rb = p.row0 + tn * kTileN2;
+                        mbar_arrive_expect_tx(&full[stage], (uint32_t)(pass ? 4 * kHalf : 2 * kHalf));
+                        tma_load_3d(dst, &mapA, k, ra, 0, &full[stage]);
+                        tma_load_3d(dst + 2 * kHalf, &mapB, k, rb, 0, &full[stage]);
+                        if (pass) {
+                            tma_load_3d(dst + kHalf, &mapA, k, ra, 4, &full[stage]);
+                            tma_load_3d(dst + 3 * kHalf, &mapB, k, rb, 4, &full[stage]);
+                        }
+                        if (++stage == kStages2) { stage = 0; phase ^= 1; }
+                    }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            int stage = 0, phase = 0, tphase = 0;
+            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                if (!oz_tile<kTileN2>(p, tile / p.tiles_n, tile % p.tiles_n).wanted) continue;
+                for (int pass = 0; pass < 2; ++pass) {
+                    mbar_wait(tmem_empty, (uint32_t)(tphase ^ 1));      // the epilogue has drained the previous four level sums
+                    tc_fence_after();
+                    for (int kc = 0; kc < p.kchunks; ++kc) {
+                        mbar_wait(&full[stage], (uint32_t)phase);
+                        tc_fence_after();
+                        const uint32_t sa = smem_u32(base + (size_t)stage * kSlotBytes2), sb = sa + 2 * kHalf;
+                        const uint32_t acc = (kc > 0) ? 1u : 0u;
+                        if (pass == 0) {
+#pragma unroll
+                            for (int pa = 0; pa < 4; ++pa)
+#pragma unroll
+                                for (int pb = 0; pb + pa < 4; ++pb)
+                                    mma_i8(tmem_base + (uint32_t)((pa + pb) * kTileN2), smem_desc_sw32(sa + pa * kPlaneBytes),
+                                           smem_desc_sw32(sb + pb * kPlaneBytes), kIdescI8N128, pa > 0 ? 1u : acc);
+                        } else {
+#pragma unroll
+                            for (int pa = 0; pa < kPlanes; ++pa)
+#pragma unroll
+                                for (int pb = 0; pb < kPlanes; ++pb)
+                                    if (pa + pb >= 4 && pa + pb < kPlanes)
+                                        mma_i8(tmem_base + (uint32_t)(((pa + pb) & 3) * kTileN2), smem_desc_sw32(sa + pa * kPlaneBytes),
+                                               smem_desc_sw32(sb + pb * kPlaneBytes), kIdescI8N128, pa > 0 ? 1u : acc);
+                        }
+                        tc_commit(&empty[stage]);
+                        if (++stage == kStages2) { stage = 0; phase ^= 1; }
+                    }
+                    tc_commit(tmem_full);
+                    tphase ^= 1;
+                }
+            }
+        }
+    } else {
+        // ===== epilogue: 4 warps, warp w owns the TMEM lanes 32 (w % 4) .. +31 = rows of the tile =====
+        const int quad = warp & 3;
+        int tphase = 0;
+        const double s2 = p.scale ? (*p.scale) * (*p.scale) : 1.0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const OzTile ot = oz_tile<kTileN2>(p, tile / p.tiles_n, tile % p.tiles_n);
+            if (!ot.wanted) continue;
+            double* crow = ot.c + (size_t)(32 * quad + lane) * ot.ld;
+            for (int pass = 0; pass < 2; ++pass) {
+                mbar_wait(tmem_full, (uint32_t)tphase);
+                tc_fence_after();
+                // weight of the LAST level of this pass (3 or 7): w_last is that of level 7, a level up weighs 128 x more
+                const double wl = p.w_last * s2 * (pass ? 1.0 : 268435456.0);       // 128^4
+#pragma unroll 1
+                for (int c0 = 0; c0 < kTileN2; c0 += 16) {
+                    double acc[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) acc[j] = 0.0;
+                    double w = wl;
+#pragma unroll
+                    for (int l = 3; l >= 0; --l) {                            // smallest weight first
+                        int32_t v[16];
+                        tmem_ld16(tmem_base + ((uint32_t)(32 * quad) << 16) + (uint32_t)(l * kTileN2 + c0), v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) acc[j] = fma((double)v[j], w, acc[j]);
+                        w *= 128.0;
+                    }
+#pragma unroll
+                    for (int j = 0; j < 16; j += 2) {
+                        double2 c = *reinterpret_cast<double2*>(crow + c0 + j);
+                        c.x -= acc[j];
+                        c.y -= acc[j + 1];
+                        *reinterpret_cast<double2*>(crow + c0 + j) = c;
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tmem_empty);
+                tphase ^= 1;
+            }
         }
     }
     tc_fence_before();

@@ -499,6 +499,7 @@ def run_b200(args):
     total_ms = sum(events[s][0].elapsed_time(events[s][5]) for s in range(args.steps))
     per_step_chol = [events[s][1].elapsed_time(events[s][2]) for s in range(args.steps)]
 
+    phase_full_cov_ms = phase["full_cov"] / args.steps
     # SURVEY.md 8(f) rows 1 and 4, outside the step (reported next to it): variance-only prediction given L and
     # the log marginal likelihood, median of 3 after one warm-up
     var = torch.empty(m, dtype=torch.float64, device="cuda")
@@ -536,6 +537,23 @@ def run_b200(args):
                     "(tcgen05.mma kind::i8, TMEM accumulators); not the headline: dtype of `value` stays f64"}
         del L64, Lmx, mwork
         pipe.assemble(dX); pipe.cholesky(); pipe.solve(dY)       # leave the FP64 factor behind for what follows
+        if m <= 65536:
+            # ... and the full-covariance prediction on the same emulated contraction (given L), beside the FP64 one
+            gp.gp_predict_full_cov(pipe.KL, dX, dXs, h, tile, args.width, pipe.Sigma, pipe.work)
+            S64 = pipe.Sigma.clone()
+            pwork = torch.empty(gp.gp_mixed_predict_workspace_bytes(n, m, tile), dtype=torch.uint8, device="cuda")
+            tpx = []
+            for r in range(4):
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                e[0].record(); gp.gp_predict_full_cov_mixed(pipe.KL, dX, dXs, h, tile, args.width, pipe.Sigma, pwork); e[1].record()
+                torch.cuda.synchronize()
+                if r > 0:
+                    tpx.append(e[0].elapsed_time(e[1]))
+            next_rows["full_cov_mixed_int8_emulated"] = {
+                "ms": statistics.median(tpx), "fp64_path_ms": phase_full_cov_ms,
+                "rel_diff_to_fp64_sigma": float((pipe.Sigma - S64).norm() / S64.norm()),
+                "what": "gp_predict_full_cov_mixed: V^T solve and W = V^T V as split-operand int8 products, TRSM with the diagonal tiles in FP64"}
+            del S64, pwork
     torch.cuda.empty_cache()
 
     # end to end through the host-buffer C-ABI call: H2D of X, y, X^ and D2H of mean, Sigma inside

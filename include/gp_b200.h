@@ -255,6 +255,16 @@ int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int
                    void* stream);
 int gp_mixed_slice_column(const double* dKL, int64_t n, int tile, int J, void* dWork, size_t work_bytes, void* stream);
 
+/* The full-covariance prediction on the same emulated contraction (opt-in; gp_predict_full_cov is unchanged): the
+ * V^T solve left-looking over tile columns (column P gets V^T(:,0:P) L(P,0:P)^T in one emulated contraction, then its FP64
+ * TRSM with the diagonal tile on the executor, then its digit planes), and W = V^T (V^T)^T in ONE emulated contraction of
+ * depth n over the lower triangle of Sigma, mirrored.  Arguments as gp_predict_full_cov; additionally tile % 128 == 0,
+ * n / tile <= 60, n <= 65536, m <= 65536.  dWork: gp_mixed_predict_workspace_bytes() (V^T and the digit planes of L and
+ * of V^T: 8 (m n + n^2 + m n) bytes). */
+int gp_mixed_predict_workspace_bytes(int64_t n, int64_t m, int tile, size_t* bytes);
+int gp_predict_full_cov_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
+                              int tile, int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream);
+
 /* Host-only replay check of the panel schedule of step J (returns the number of work items, or a negative GP_ERR_*). */
 int gp_panel_schedule_selfcheck(int64_t n, int tile, int J);
 

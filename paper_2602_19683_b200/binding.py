@@ -28,7 +28,8 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
-           "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n")
+           "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n",
+           "gp_mixed_predict_workspace_bytes", "gp_predict_full_cov_mixed")
 
 
 class gp_hyper(ctypes.Structure):
@@ -102,6 +103,8 @@ def load() -> ctypes.CDLL:
     lib.gp_mixed_slice_column.argtypes = [vp, i64, ci, ci, vp, sz, vp]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
     lib.gp_set_ozaki_tile_n.argtypes = [ci]
+    lib.gp_mixed_predict_workspace_bytes.argtypes = [i64, i64, ci, psz]
+    lib.gp_predict_full_cov_mixed.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
     lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
     lib.gp_block_size_for.argtypes = [i64, ci]
@@ -349,6 +352,20 @@ def gp_mixed_slice_column(KL: torch.Tensor, n: int, tile: int, J: int, work: tor
 
 def gp_panel_schedule_selfcheck(n: int, tile: int, J: int) -> int:
     return int(load().gp_panel_schedule_selfcheck(n, tile, J))
+
+
+def gp_mixed_predict_workspace_bytes(n: int, m: int, tile: int) -> int:
+    b = ctypes.c_size_t(0)
+    _check(load().gp_mixed_predict_workspace_bytes(n, m, tile, ctypes.byref(b)), "gp_mixed_predict_workspace_bytes")
+    return int(b.value)
+
+
+def gp_predict_full_cov_mixed(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
+                              Sigma: torch.Tensor, work: torch.Tensor) -> None:
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_full_cov_mixed(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(Sigma),
+                                            _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_full_cov_mixed")
 
 
 def gp_set_ozaki_tile_n(n: int) -> None:

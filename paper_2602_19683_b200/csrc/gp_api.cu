@@ -1045,11 +1045,11 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     q.kchunks = (int)((int64_t)(k_tile1 - k_tile0) * tile / oz::kChunk);
     q.kc0 = (int)((int64_t)k_tile0 * tile / oz::kChunk);
     q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
-    q.scale = (const double*)(c.ws + c.w.scale);
+    q.scale = (const double*)(c.ws + c.w.scale) + 1;          // scale^2
     q.tiled = 1;
     q.t = tile;
     q.J = J;
-    q.row0 = J * tile;
+    q.row0a = q.row0b = J * tile;
     // both operands come from the dense digit planes [8][n][n] of the whole matrix
     return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, c.st);
 }
@@ -1112,6 +1112,145 @@ extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sch
         if ((rc = gp_mixed_slice_column(dKL, n, tile, J, dWork, work_bytes, stream)) != GP_OK) return rc;
     }
     return GP_OK;
+}
+
+// ---- the prediction on the same emulated contraction (continued) ---------------------------------
+namespace {
+struct MixedPredWs { size_t ticket, verV, invD, items, scale, Vt, planesL, planesV, total; };
+MixedPredWs mixed_pred_ws(int64_t n, int64_t m) {
+    const size_t NB = (size_t)(n / 128), NBm = (size_t)(m / 128);
+    MixedPredWs w;
+    w.ticket = 0;
+    w.verV = kHdrBytes;
+    w.invD = align_up(w.verV + NBm * NB * sizeof(int), 256);
+    w.items = align_up(w.invD + NB * (size_t)128 * 128 * sizeof(double), 256);
+    w.scale = align_up(w.items + NBm * sizeof(Item), 256);
+    w.Vt = align_up(w.scale + 256, 1024);
+    w.planesL = align_up(w.Vt + (size_t)m * (size_t)n * sizeof(double), 1024);
+    w.planesV = align_up(w.planesL + (size_t)oz::kPlanes * (size_t)n * (size_t)n, 1024);
+    w.total = w.planesV + (size_t)oz::kPlanes * (size_t)m * (size_t)n;
+    return w;
+}
+}  // namespace
+
+extern "C" int gp_mixed_predict_workspace_bytes(int64_t n, int64_t m, int tile, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    int rc = mixed_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m <= 0 || m > 65536) return GP_ERR_SIZE;
+    if ((rc = tile_ok(m, tile)) != GP_OK) return rc;
+    *bytes = mixed_pred_ws(n, m).total;
+    return GP_OK;
+}
+
+extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
+                                         int tile, int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
+    if (!dL || !dX || !dXs || !dSigma || !dWork) return GP_ERR_NULL;
+    int rc = mixed_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (m <= 0 || m > 65536 || D <= 0) return GP_ERR_SIZE;
+    if ((rc = tile_ok(m, tile)) != GP_OK) return rc;
+    if (!hyper_ok(h)) return GP_ERR_HYPER;
+    const MixedPredWs w = mixed_pred_ws(n, m);
+    if (work_bytes < w.total) return GP_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    constexpr int b = 128;
+    const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
+    char* ws = (char*)dWork;
+    double* Vt = (double*)(ws + w.Vt);
+    double* invD = (double*)(ws + w.invD);
+    double* scale = (double*)(ws + w.scale);                          // [sL, sV, sL sV, sV sV], then the bits of max |L|
+    unsigned long long* maxbits = (unsigned long long*)(scale + 8);
+    int8_t* planesL = (int8_t*)(ws + w.planesL);
+    int8_t* planesV = (int8_t*)(ws + w.planesV);
+    Item* items = (Item*)(ws + w.items);
+    const HyperDev hd = to_dev(h);
+    if (cudaMemsetAsync(ws, 0, w.invD, st) != cudaSuccess) return GP_ERR_CUDA;
+    if (cudaMemsetAsync(scale, 0, 256, st) != cudaSuccess) return GP_ERR_CUDA;
+    // a9: K_{X^,X} straight into V^T, the prior K_{X^,X^} straight into Sigma (as gp_predict_full_cov)
+    if ((rc = launch_assemble(dXs, m, dX, n, D, hd, tile, 0, Vt, st)) != GP_OK) return rc;
+    {
+        const int sb = (int)((m + kAsmBlk - 1) / kAsmBlk);
+        const size_t smem = 2 * (size_t)kAsmMaxD * kAsmBlk * sizeof(double);
+        assemble_tiles_kernel<<<(unsigned)(sb * sb), 256, smem, st>>>(dXs, dXs, D, hd, (int)m, 1, 0, dSigma);
+        if (cudaGetLastError() != cudaSuccess) return GP_ERR_CUDA;
+    }
+    if ((rc = launch_trtri_any(b, dL, tile, NB, invD, st)) != GP_OK) return rc;
+    // fixed-point scales: |L_ij| <= max |L| (read from the factor), |V_ia| <= sqrt(k(x^_a, x^_a)) = sqrt(v)
+    const double sv = std::ldexp(1.0, (int)std::ceil(std::log2(std::sqrt(h.vertical))) + 1);
+    const int64_t lcount = (int64_t)M * (M + 1) / 2 * tile * tile;
+    oz::absmax_lower_tiles_kernel<<<sm_count() * 8, 256, 0, st>>>(dL, lcount, maxbits);
+    oz::finish_scales_kernel<<<1, 1, 0, st>>>(maxbits, sv, scale);
+    for (int J = 0; J + 1 < M; ++J) {                                 // digit planes of the factor (tiles below the diagonal tiles)
+        const int64_t total = (n - (int64_t)(J + 1) * tile) * (tile / 4);
+        const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
+        oz::slice_tile_column_kernel<<<grid, 256, 0, st>>>(dL, n, tile, J, scale, planesL);
+    }
+    ExecParams p;
+    memset(&p, 0, sizeof(p));
+    p.L = const_cast<double*>(dL);
+    p.Vt = Vt;
+    p.invD = invD;
+    p.verV = (int*)(ws + w.verV);
+    p.verS = p.verV;
+    p.items = items;
+    p.nitems = NBm;
+    p.stats = (unsigned long long*)(ws + kStatsOff);
+    p.t = tile;
+    p.nbt = nbt;
+    p.snbt = nbt;
+    p.NB = NB;
+    p.NBm = NBm;
+    p.Mt = M;
+    p.m = m;
+    p.L_final = 1;
+    ExecMaps mp;
+    if ((rc = make_exec_maps(&mp, p, b, m)) != GP_OK) return rc;
+    for (int P = 0; P < M; ++P) {
+        if (P > 0) {
+            // left-looking: V^T(:, P) -= V^T(:, 0:P) L(P, 0:P)^T, one emulated contraction of depth P * tile
+            oz::OzParams q;
+            memset(&q, 0, sizeof(q));
+            q.C = Vt;
+            q.tiles_m = (int)(m / oz::kTileM);
+            q.kchunks = (int)((int64_t)P * tile / oz::kChunk);
+            q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+            q.scale = scale + 2;
+            q.tiled = 2;
+            q.t = tile;
+            q.J = P;
+            q.Mt = M;
+            q.row0a = 0;
+            q.row0b = P * tile;
+            if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesL, (uint64_t)n, (uint64_t)n, tile, st)) != GP_OK) return rc;
+        }
+        // the FP64 half of step P: V^T(:, P) <- V^T(:, P) L(P,P)^-T, one ROW_V chain per block row, on the executor
+        oz::set_general_column_versions_kernel<<<(NBm * nbt + 255) / 256, 256, 0, st>>>(p.verV, NBm, NB, nbt, P, kConsumerWarps);
+        cov_row_items_kernel<<<(NBm + 255) / 256, 256, 0, st>>>((uint4*)items, NBm, 0, 1, 0, (unsigned)OP_ROW_V);
+        row_items_set_column_kernel<<<(NBm + 255) / 256, 256, 0, st>>>((uint4*)items, NBm, (unsigned)(P * nbt));
+        p.ticket = (unsigned int*)(ws + w.ticket) + P;
+        if ((rc = launch_exec<128>(p, mp, workers_for(sched_width), st)) != GP_OK) return rc;
+        {
+            const int64_t total = m * (tile / 4);
+            const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
+            oz::slice_general_column_kernel<<<grid, 256, 0, st>>>(Vt, m, n, tile, P, scale + 1, planesV);
+        }
+    }
+    {   // a12: Sigma -= V^T (V^T)^T over the lower triangle, one emulated contraction of depth n; then the mirror
+        oz::OzParams q;
+        memset(&q, 0, sizeof(q));
+        q.C = dSigma;
+        q.ldc = m;
+        q.tiles_m = (int)(m / oz::kTileM);
+        q.kchunks = (int)(n / oz::kChunk);
+        q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+        q.scale = scale + 3;
+        q.tiled = 3;
+        if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesV, (uint64_t)m, (uint64_t)n, m, st)) != GP_OK) return rc;
+    }
+    dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
+    mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
 extern "C" int gp_panel_schedule_selfcheck(int64_t n, int tile, int J) {

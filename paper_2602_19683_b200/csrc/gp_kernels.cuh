@@ -192,6 +192,17 @@ __global__ void cov_row_items_kernel(uint4* __restrict__ items, int rows, int gr
         items[idx] = make_uint4(op, (unsigned)(gr0 + idx / NBm), (unsigned)(idx % NBm), (unsigned)NB << 16);
 }
 
+// ROW_V items of one tile column: item i = (op, gr = i, gc = first block column of the tile column, 0)
+__global__ void row_items_set_column_kernel(uint4* __restrict__ items, int rows, unsigned gc) {
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < rows; idx += gridDim.x * blockDim.x) {
+        uint4 it = items[idx];
+        it.y = (unsigned)idx;
+        it.z = gc;
+        it.w = 0u;
+        items[idx] = it;
+    }
+}
+
 // tiles -> dense (inspection helper)
 __global__ void tiles_to_dense_kernel(const double* __restrict__ tiles, int64_t n, int64_t nb, int tile, int lower_packed,
                                       double* __restrict__ dense) {

@@ -124,8 +124,69 @@ __global__ void __launch_bounds__(1024) factor_scale_kernel(const double* __rest
         for (int k = 0; k < 32; ++k) m = fmax(m, s_max[k]);
         int e;
         const double f = frexp(sqrt(m > 0.0 ? m : 1.0), &e);      // sqrt(m) = f 2^e, f in [0.5, 1)
-        *scale = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0));          // >= 2 sqrt(m), with a little head-room at the edge
+        const double sc = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0)); // >= 2 sqrt(m), with a little head-room at the edge
+        scale[0] = sc;
+        scale[1] = sc * sc;                                          // the weight factor of a product of two such operands
     }
+}
+
+// The same from a FINISHED factor: scale[0] <- power of two >= 2 max |L_ij| (lower tiles), scale[1] <- sv (given),
+// scale[2] <- scale[0] * sv, scale[3] <- sv * sv.  Two launches: a grid-wide maximum (positive doubles order like their
+// bit patterns), then the finish.
+__global__ void __launch_bounds__(256) absmax_lower_tiles_kernel(const double* __restrict__ tiles, int64_t count, unsigned long long* __restrict__ bits) {
+    double m = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (int64_t)gridDim.x * blockDim.x) m = fmax(m, fabs(tiles[i]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m == m) atomicMax(bits, (unsigned long long)__double_as_longlong(m));
+}
+__global__ void finish_scales_kernel(const unsigned long long* __restrict__ bits, double sv, double* __restrict__ scale) {
+    const double m = __longlong_as_double((long long)*bits);
+    int e;
+    const double f = frexp(m > 0.0 ? m : 1.0, &e);
+    const double sl = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0));
+    scale[0] = sl;
+    scale[1] = sv;
+    scale[2] = sl * sv;
+    scale[3] = sv * sv;
+}
+
+// tile column J of a GP_GENERAL tiled m x n matrix (all tile rows) -> dense planes [p][m][n]
+__global__ void __launch_bounds__(256) slice_general_column_kernel(const double* __restrict__ tiles, int64_t m, int64_t n, int t, int J,
+                                                                   const double* __restrict__ scale, int8_t* __restrict__ planes) {
+    const double inv_scale = 1.0 / *scale;
+    const int64_t total = m * (t / 4);
+    const int64_t Mt = n / t;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t gi = idx / (t / 4);
+        const int c = 4 * (int)(idx % (t / 4));
+        const int64_t a = gi / t, r = gi % t;
+        const double* src = tiles + ((size_t)a * Mt + J) * (size_t)t * t + (size_t)r * t + c;
+        const double2 v01 = *reinterpret_cast<const double2*>(src), v23 = *reinterpret_cast<const double2*>(src + 2);
+        const double xs[4] = {v01.x, v01.y, v23.x, v23.y};
+        uint32_t packed[kPlanes];
+#pragma unroll
+        for (int p = 0; p < kPlanes; ++p) packed[p] = 0u;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            long long I56 = __double2ll_rn(xs[e] * inv_scale * 72057594037927936.0);
+#pragma unroll
+            for (int p = kPlanes - 1; p >= 0; --p) {
+                const long long d = ((I56 + 64) & 127) - 64;
+                I56 = (I56 - d) >> kDigitBits;
+                packed[p] |= (uint32_t)((int)d & 0xff) << (8 * e);
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < kPlanes; ++p)
+            *reinterpret_cast<uint32_t*>(planes + ((size_t)p * m + gi) * n + (size_t)J * t + c) = packed[p];
+    }
+}
+
+// version counters of the blocks of tile column J of V^T <- "J updates applied"
+__global__ void set_general_column_versions_kernel(int* __restrict__ ver, int NBm, int NB, int nbt, int J, int per_version) {
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < NBm * nbt; idx += gridDim.x * blockDim.x)
+        ver[(size_t)(idx / nbt) * NB + J * nbt + idx % nbt] = J * per_version;
 }
 
 // version counters of the blocks of tile column J <- "J trailing updates applied" (they were applied by the emulated
@@ -194,11 +255,13 @@ struct OzParams {
     int64_t ldc;
     int tiles_m, tiles_n, kchunks;
     double w_last;        // scaleA * scaleB * 2^(-7 (S + 1)): weight of level S - 1; level l weighs scaleA scaleB 2^(-7 (l + 2))
-    const double* scale;  // optional device scalar s: the weights are multiplied by s^2 (operands sliced with a scale found on the device)
-    // tiled mode (gp_cholesky_tiled_mixed): the output is tile column J of a lower-packed matrix of t x t tiles, rows from
-    // tile row J down; operand rows and the k extent are taken from dense digit planes of the whole matrix
-    int tiled, t, J;
-    int row0;             // first operand row of A and of B in the planes (J * t)
+    const double* scale;  // optional device scalar: the weights are multiplied by it (= scaleA * scaleB of operands that were
+                          // sliced with scales found on the device)
+    // output modes:  0 dense C (ldc);  1 tile column J of a LOWER-PACKED matrix of t x t tiles, rows from tile row J down
+    // (gp_cholesky_tiled_mixed);  2 tile column J of a GP_GENERAL matrix with Mt tile columns, all tile rows (the V^T solve);
+    // 3 dense C, only the 128 x TN pieces that touch the lower triangle (Sigma)
+    int tiled, t, J, Mt;
+    int row0a, row0b;     // first operand row of A and of B in their digit planes
     int kc0;              // first k-chunk (the contraction covers the chunks [kc0, kc0 + kchunks))
 };
 
@@ -211,13 +274,20 @@ struct OzTile {
 template <int TN = kTileN>
 __device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
     OzTile o;
-    if (!p.tiled) {
-        o.wanted = true;
+    if (p.tiled == 0 || p.tiled == 3) {
+        o.wanted = p.tiled == 0 || tn * TN < (tm + 1) * kTileM;
         o.ld = p.ldc;
         o.c = p.C + (size_t)tm * kTileM * p.ldc + (size_t)tn * TN;
         return o;
     }
     const int bpt = p.t / kTileM;                       // 128-row blocks per tile edge
+    if (p.tiled == 2) {
+        const int a = tm / bpt, rblk = tm % bpt;
+        o.wanted = true;
+        o.ld = p.t;
+        o.c = p.C + ((size_t)a * p.Mt + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * TN;
+        return o;
+    }
     const int I = p.J + tm / bpt, rblk = tm % bpt;
     // on the diagonal tile only the lower part is data: skip 128 x TN pieces that lie wholly above the diagonal
     o.wanted = !(I == p.J && tn * TN >= (rblk + 1) * kTileM);
@@ -262,8 +332,8 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
                     mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
                     char* dst = base + (size_t)stage * kStageBytesOz;
                     mbar_arrive_expect_tx(&full[stage], (uint32_t)kStageBytesOz);
-                    tma_load_3d(dst, &mapA, (p.kc0 + kc) * kChunk, p.row0 + tm * kTileM, 0, &full[stage]);
-                    tma_load_3d(dst + kABytes, &mapB, (p.kc0 + kc) * kChunk, p.row0 + tn * kTileN, 0, &full[stage]);
+                    tma_load_3d(dst, &mapA, (p.kc0 + kc) * kChunk, p.row0a + tm * kTileM, 0, &full[stage]);
+                    tma_load_3d(dst + kABytes, &mapB, (p.kc0 + kc) * kChunk, p.row0b + tn * kTileN, 0, &full[stage]);
                     if (++stage == kStagesOz) { stage = 0; phase ^= 1; }
                 }
             }
@@ -307,7 +377,7 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
             mbar_wait(tmem_full, (uint32_t)tphase);
             tc_fence_after();
             double* crow = ot.c + (size_t)(32 * quad + lane) * ot.ld;
-            const double wl = p.scale ? p.w_last * (*p.scale) * (*p.scale) : p.w_last;
+            const double wl = p.scale ? p.w_last * (*p.scale) : p.w_last;
 #pragma unroll 1
             for (int c0 = 0; c0 < kTileN; c0 += 16) {
                 double acc[16];
@@ -401,7 +471,7 @@ ozaki_contract_kernel2(const __grid_constant__ OzParams p, const __grid_constant
                     for (int kc = 0; kc < p.kchunks; ++kc) {
                         mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
                         char* dst = base + (size_t)stage * kSlotBytes2;
-                        const int k = (p.kc0 + kc) * kChunk, ra = p.row0 + tm * kTileM, rb = p.row0 + tn * kTileN2;
+                        const int k = (p.kc0 + kc) * kChunk, ra = p.row0a + tm * kTileM, rb = p.row0b + tn * kTileN2;
                         mbar_arrive_expect_tx(&full[stage], (uint32_t)(pass ? 4 * kHalf : 2 * kHalf));
                         tma_load_3d(dst, &mapA, k, ra, 0, &full[stage]);
                         tma_load_3d(dst + 2 * kHalf, &mapB, k, rb, 0, &full[stage]);
@@ -455,7 +525,7 @@ ozaki_contract_kernel2(const __grid_constant__ OzParams p, const __grid_constant
         // ===== epilogue: 4 warps, warp w owns the TMEM lanes 32 (w % 4) .. +31 = rows of the tile =====
         const int quad = warp & 3;
         int tphase = 0;
-        const double s2 = p.scale ? (*p.scale) * (*p.scale) : 1.0;
+        const double s2 = p.scale ? (*p.scale) : 1.0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const OzTile ot = oz_tile<kTileN2>(p, tile / p.tiles_n, tile % p.tiles_n);
             if (!ot.wanted) continue;

@@ -118,3 +118,31 @@ def test_mixed_cholesky_reports_a_non_positive_pivot(gp):
     gp.gp_cholesky_tiled_mixed(KL, n, tile, 0, info, work)
     torch.cuda.synchronize()
     assert int(info.item()) == 301
+
+
+@pytest.mark.parametrize("n,m,D,tile", [(512, 256, 8, 128), (1024, 512, 8, 256), (2048, 1024, 5, 512), (1536, 256, 8, 256)])
+def test_mixed_prediction_matches_oracle(gp, n, m, D, tile):
+    """gp_predict_full_cov_mixed (V^T solve and W on the emulated contraction, TRSM with the diagonal tiles in FP64) on the
+    factor of gp_cholesky_tiled_mixed: Sigma against the oracle at north_star's 1e-9, exactly symmetric."""
+    from paper_2602_19683_b200 import nfir
+    X, y = nfir.nfir_features(3 * n + m, n, D)
+    Xs, _ = nfir.nfir_features(5 * n + m, m, D, with_targets=False)
+    h = oracle.Hyper(1.0, 1.3, 0.1)
+    p = oracle.predict(X, y, Xs, h)
+    hg = gp.Hyper(1.0, 1.3, 0.1)
+    pipe = gp.GpPipeline(n, m, D, tile, hg)
+    dX, dXs = torch.from_numpy(X).cuda(), torch.from_numpy(Xs).cuda()
+    pipe.assemble(dX)
+    work = torch.empty(max(gp.gp_mixed_workspace_bytes(n, tile), gp.gp_mixed_predict_workspace_bytes(n, m, tile)), dtype=torch.uint8, device="cuda")
+    gp.gp_cholesky_tiled_mixed(pipe.KL, n, tile, 0, pipe.info, work)
+    gp.gp_predict_full_cov_mixed(pipe.KL, dX, dXs, hg, tile, 0, pipe.Sigma, work)
+    torch.cuda.synchronize()
+    assert int(pipe.info.item()) == 0
+    S = pipe.Sigma.cpu().numpy()
+    err = relerr(S, p.Sigma)
+    print(f"mixed prediction n={n} m={m} tile={tile}: |Sigma - Sigma_oracle| / |Sigma_oracle| = {err:.2e}")
+    assert err <= 1e-9
+    np.testing.assert_allclose(S, p.Sigma, rtol=0, atol=1e-9 * np.abs(p.Sigma).max())
+    assert np.array_equal(S, S.T)
+    d = np.diag(S)
+    assert d.min() >= 0.0 and d.max() <= h.vertical

@@ -91,7 +91,7 @@ struct Cost {
     double per_q, fixed, potrf;
     explicit Cost(int blk) {
         if (blk >= 128) { per_q = 17.6; fixed = 2.5; potrf = 40.0; }     // potrf: the r02 diagonal block (38 us measured)
-        else if (blk >= 64) { per_q = 3.6; fixed = 3.0; potrf = 16.0; }
+        else if (blk >= 64) { per_q = 2.6; fixed = 3.0; potrf = 16.0; }     // per_q: n = 8192 runs at <= 3.05 us per 64^3 product all in
         else { per_q = 0.8; fixed = 2.5; potrf = 7.0; }
     }
     double of(const SchedItem& it, int nbt) const {

@@ -848,41 +848,44 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
 
 // ---- split-operand (Ozaki) contraction on the int8 tensor cores -------------------------
 namespace {
-// planes [S][rows][k] (int8) viewed through boxes of {32 bytes of k, box_rows rows, all S planes}, 32-byte swizzle
-int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64_t k, uint32_t box_rows, uint32_t box_planes = oz::kPlanes) {
+// planes [S][rows][k] (int8) viewed through boxes of {chunk bytes of k, box_rows rows, box_planes planes}; the swizzle is as
+// wide as the box row (32 bytes: all planes of a k-chunk per box; 128 bytes: one plane per box)
+int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64_t k, uint32_t box_rows, uint32_t box_planes = oz::kPlanes,
+                   uint32_t chunk = oz::kChunk) {
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return GP_ERR_CUDA;
     const cuuint64_t dims[3] = {(cuuint64_t)k, (cuuint64_t)rows, (cuuint64_t)oz::kPlanes};
     const cuuint64_t strides[2] = {(cuuint64_t)k, (cuuint64_t)(rows * k)};
-    const cuuint32_t box[3] = {(cuuint32_t)oz::kChunk, box_rows, box_planes};
+    const cuuint32_t box[3] = {chunk, box_rows, box_planes};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<int8_t*>(planes), dims, strides, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, chunk == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_32B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? GP_OK : GP_ERR_CUDA;
 }
 }  // namespace
 
 namespace {
-std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (= 64: see gp_ozaki.cuh), 64, 128: gp_set_ozaki_tile_n (measurement support)
+std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (128 when the shape allows), 64, 128: gp_set_ozaki_tile_n (measurement support)
 
-// launches the emulated contraction described by q (tiles_n counted in 64-column units on entry) with the chosen tile shape
+// launches the emulated contraction described by q (kc0 / kchunks in 32-byte chunks) with the tile shape that fits:
+// the 128 x 128 two-pass kernel when the column count and the k range are multiples of 128, else the 128 x 64 one
 int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const int8_t* planesB, uint64_t rowsB, uint64_t kdim, int64_t ncols,
                  cudaStream_t st) {
     const int want = g_ozaki_tile_n.load(std::memory_order_relaxed);
-    const bool wide = want == 128 && ncols % oz::kTileN2 == 0;
+    const bool wide = want != 64 && ncols % oz::kTileN3 == 0 && q.kchunks % oz::kKSteps3 == 0 && q.kc0 % oz::kKSteps3 == 0 && kdim % oz::kChunk3 == 0;
     CUtensorMap mapA, mapB;
     int rc;
     if (wide) {
-        if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM, 4)) != GP_OK) return rc;
-        if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN2, 4)) != GP_OK) return rc;
+        if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM, 1, oz::kChunk3)) != GP_OK) return rc;
+        if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN3, 1, oz::kChunk3)) != GP_OK) return rc;
         rc = configure_once(1024u, [] {
-            return cudaFuncSetAttribute(oz::ozaki_contract_kernel2, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz2) == cudaSuccess;
+            return cudaFuncSetAttribute(oz::ozaki_contract_kernel3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz3) == cudaSuccess;
         });
         if (rc != GP_OK) return rc;
-        q.tiles_n = (int)(ncols / oz::kTileN2);
+        q.tiles_n = (int)(ncols / oz::kTileN3);
         const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
-        oz::ozaki_contract_kernel2<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz2, st>>>(q, mapA, mapB);
+        oz::ozaki_contract_kernel3<0><<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB);
     } else {
         if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM)) != GP_OK) return rc;
         if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN)) != GP_OK) return rc;

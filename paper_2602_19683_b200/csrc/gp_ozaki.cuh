@@ -233,6 +233,14 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t (&v)[16]) {
         : "r"(taddr)
         : "memory");
 }
+// one lane of a converged warp; the loops of the wide kernel are run by WHOLE warps with the side effects under this
+// predicate: code under `if (lane == 0)` makes ptxas treat every operand as divergent and wrap each tcgen05.mma in an
+// R2UR + ELECT + BRA.U.ANY loop, code that is uniform across the warp keeps descriptors in uniform registers
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n .reg .pred P;\n elect.sync _|P, 0xffffffff;\n selp.u32 %0, 1, 0, P;\n}\n" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
 
 __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
@@ -413,40 +421,193 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
 }
 
 
-// ---- second shape: 128 x 128 output tile, the eight levels in TWO passes of four ---------------------------------------
-// The 128 x 64 kernel above keeps all eight level sums in tensor memory, so every operand byte is fetched once -- but each
-// of its MMAs (128 x 64 x 32) makes the tensor core read 4 KB of A and 2 KB of B from shared memory for 32 cycles of
-// work: 192 B/cycle against a shared-memory port of 128 B/cycle.  With N = 128 an MMA reads 4 + 4 KB for 64 cycles
-// (128 B/cycle), and tensor memory holds four level sums of 128 columns: the levels are done in two passes over k
-// (levels 0-3 need the planes 0-3 only: 10 products per chunk; levels 4-7 need all planes: 26), which costs exactly the
-// L2 traffic the 128 x 64 kernel spends on loading A once per column half.
-// MEASURED (8192 x 8192 x k, FP64-equivalent TFLOP/s): k = 1024 / 4096 / 16384: 128 x 64: 59.7 / 63.4 / 64.7;
-// 128 x 128: 51.8 / 68.1 / 62.7.  The two shapes end at the same 2.3-2.45 int8 POPS although their shared-memory
-// demand differs by a third: what they share is the 96 KB per 128 x 128 x 32 product that travel from L2 to shared
-// memory (5.9 TB/s over the chip at that rate), so that, not the operand read of the tensor core, is the bound.  The
-// way past it is a larger output tile per operand byte (a CTA pair with cta_group::2 / TMA multicast); not built.
-// The 128 x 64 shape is the default (no second pass, so no drain bubble at short k).
-constexpr int kTileN2 = 128;
-constexpr int kSlotBytes2 = 2 * kPlanes * kTileM * kChunk;          // 64 KB: 8 planes of A + 8 planes of B, one k-chunk
-constexpr int kStages2 = 3;
-constexpr int kSmemOz2 = kStages2 * kSlotBytes2 + 1024 + 256;
-constexpr uint32_t kIdescI8N128 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTileN2 >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+// ---- the wide shape: 128 x 128 output tile, 128-byte k-chunks, the levels in TWO passes --------------------------------
+// What bounds the 128 x 64 kernel above was measured with probes (profiles/r02_ozaki_bounds.md): with the TMA loads
+// removed it runs at the SAME rate, so it is not the operand stream from L2; a bare issue loop shows that a
+// tcgen05.mma kind::i8 of 128 x 64 x 32 takes 48 cycles, not 32 -- every MMA re-reads its 4 KB A operand and 2 KB B
+// operand from shared memory, 192 B/clk against a port of 128 B/clk -- while 128 x 128 x 32 takes 64 cycles = the
+// full 8192 MAC/clk/SM.  So N must be 128, and then tensor memory (512 columns) holds four level sums, not eight:
+// the levels are done in two passes over k (pass 0: the high levels, which need the leading planes only; pass 1:
+// the rest).  The first two-pass kernel (round 2, removed) kept a whole 32-byte k-chunk of ALL planes per stage and
+// was bound by the L2 -> shared-memory stream instead: TMA boxes with 32-byte rows move 9 TB/s over the chip,
+// boxes with 128-byte rows 20-29 TB/s (same probe file).  This kernel therefore streams ONE plane of ONE operand
+// per slot (128 rows x 128 bytes of k, 128-byte swizzle, 16 KB) through two rings:
+//   * step pa of a k-chunk multiplies plane pa of A with the planes pb of B whose level pa + pb lies in the pass's
+//     range [LO, HI]: a window of at most four B planes that slides down by one plane per step.  A planes live for
+//     one step, B planes are loaded in the order HI, HI-1, ... 0 and retire in the same order: both rings are FIFOs
+//     (5 A slots, 8 B slots), each with its own producer warp, so the operands of a step are requested at least
+//     2500 cycles before the step is issued;
+//   * per step up to 4 x 4 MMAs (128 x 128 x 32 each, the k-steps of a chunk address 32-byte columns of the
+//     swizzled rows); tcgen05.commit retires the A slot and the B plane that leaves the window;
+//   * epilogue by eight warps (two per TMEM lane quarter, 64 columns each): the pass's level sums -> FP64, smallest
+//     weight first, C -= result.  Pass 0 and pass 1 both update C in place.
+constexpr int kTileN3 = 128;
+constexpr int kChunk3 = 128;                                   // bytes of k per slot
+constexpr int kKSteps3 = kChunk3 / kChunk;                      // MMAs (K = 32) per plane pair and chunk
+constexpr int kSlotBytes3 = kTileM * kChunk3;                   // 16 KB
+constexpr int kNA3 = 5, kNB3 = 8;
+constexpr int kThreads3 = 352;                                  // warp 0 A producer, 1 MMA issuer, 2-9 epilogue, 10 B producer
+constexpr int kSmemOz3 = (kNA3 + kNB3) * kSlotBytes3 + 1024 + 512;
+constexpr uint32_t kIdescI8N128 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTileN3 >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 
-// map4: boxes of {32 bytes of k, 128 rows, 4 planes} (the same box serves A and B)
-__global__ void __launch_bounds__(kThreadsOz, 1)
-ozaki_contract_kernel2(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
+// the level range of a pass
+__host__ __device__ constexpr int oz3_lo(int pass) { return pass == 0 ? 0 : kPlanes / 2; }
+__host__ __device__ constexpr int oz3_hi(int pass) { return pass == 0 ? kPlanes / 2 - 1 : kPlanes - 1; }
+
+// K-major operand whose rows are 128 bytes written by TMA with the 128-byte swizzle (8-row atoms of 1024 B)
+__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
+    return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void mma_i8_n128(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t accumulate) {
+    mma_i8(tmem_d, desc_a, desc_b, kIdescI8N128, accumulate);
+}
+
+__device__ long long g_oz3_probe[16];      // PROBE == 3 only: time stamps of CTA 0's first tile
+
+struct Oz3Smem {
+    char* slotA;
+    char* slotB;
+    uint64_t *fullA, *emptyA, *fullB, *emptyB, *tmem_full, *tmem_empty;
+};
+
+// issuer: one pass over the k range for one tile.  The tensor core's instruction queue is about two MMAs deep (a pause
+// of more than ~100 cycles in the issuing thread is a bubble in the pipe: profiles/r02_ozaki_bounds.md), so the
+// mbarrier waits of the NEXT step are interleaved with the last MMAs of the current one, and a step's descriptors
+// are one add away from two per-ring base words.
+template <int LO, int HI, int PROBE>
+__device__ __forceinline__ void oz3_issue_pass(const Oz3Smem& sm, uint32_t tmem_base, int nchunks, uint32_t& cntA, uint32_t& cntB, bool leader) {
+    constexpr int QMAX = HI < kPlanes - 1 ? HI : kPlanes - 1;       // B planes QMAX .. 0 and A planes 0 .. QMAX take part
+    constexpr uint64_t kDescHi = ((uint64_t)(1024 >> 4) | ((uint64_t)1 << 14) | ((uint64_t)2 << 29)) << 32;   // SBO, version, SWIZZLE_128B
+    const uint32_t a_lo0 = ((smem_u32(sm.slotA) >> 4) & 0x3fffu) | (1u << 16);
+    const uint32_t b_lo0 = ((smem_u32(sm.slotB) >> 4) & 0x3fffu) | (1u << 16);
+    // B planes first used by step 0 of a chunk, and the A plane of a step
+    auto wait_b = [&](uint32_t cb, int q) { const uint32_t c = cb + (uint32_t)(QMAX - q); mbar_wait(&sm.fullB[c % kNB3], (c / kNB3) & 1u); };
+    auto wait_a = [&](uint32_t ca) { mbar_wait(&sm.fullA[ca % kNA3], (ca / kNA3) & 1u); };
+    // prologue: the operands of step 0 of chunk 0
+#pragma unroll
+    for (int q = QMAX; q >= 0; --q)
+        if (LO - q <= 0) wait_b(cntB, q);
+    wait_a(cntA);
+    for (int kc = 0; kc < nchunks; ++kc) {
+        const bool more = kc + 1 < nchunks;
+#pragma unroll
+        for (int pa = 0; pa <= QMAX; ++pa) {
+            tc_fence_after();
+            const uint32_t sa_slot = cntA % kNA3;
+            const uint32_t a_lo = a_lo0 + sa_slot * (uint32_t)(kSlotBytes3 >> 4);
+            // this step's MMAs: pb in [max(0, LO - pa), min(S - 1, HI - pa)], 4 k-steps each
+            const int pb_lo = LO - pa > 0 ? LO - pa : 0, pb_hi = HI - pa < kPlanes - 1 ? HI - pa : kPlanes - 1;
+            const int n_mma = (pb_hi - pb_lo + 1) * kKSteps3;
+            // waits owed to the NEXT step: (pa + 1 of this chunk) or (step 0 of the next chunk)
+            const bool wrap = pa == QMAX;
+            const int n_wait = wrap ? (QMAX - (LO > 0 ? LO : 0) + 1) + 1 : ((LO - (pa + 1) >= 0) ? 2 : 1);
+            auto next_wait = [&](int j) {            // j-th wait owed to the next step; the A plane comes last
+                if (!wrap) {
+                    if (LO - (pa + 1) >= 0) { if (j == 0) wait_b(cntB, LO - (pa + 1)); else wait_a(cntA + 1); }
+                    else wait_a(cntA + 1);
+                } else if (more) {
+                    if (j < n_wait - 1) wait_b(cntB + QMAX + 1, QMAX - j); else wait_a(cntA + 1);
+                }
+            };
+#pragma unroll
+            for (int j = 0; j < n_wait - n_mma; ++j) next_wait(j);          // more waits than MMAs: the surplus first
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {                                    // the window holds at most four B planes
+                const int pb = pb_lo + w;
+                if (pb > pb_hi) continue;
+                const uint32_t cb = cntB + (uint32_t)(QMAX - pb);
+                const uint32_t b_lo = b_lo0 + (cb % kNB3) * (uint32_t)(kSlotBytes3 >> 4);
+#pragma unroll
+                for (int ks = 0; ks < kKSteps3; ++ks) {
+                    const int m = w * kKSteps3 + ks;
+                    if (PROBE != 2 && leader)
+                        mma_i8_n128(tmem_base + (uint32_t)((pa + pb - LO) * kTileN3), kDescHi | (a_lo + ks * (kChunk >> 4)), kDescHi | (b_lo + ks * (kChunk >> 4)),
+                                    (kc > 0 || pa > 0 || ks > 0) ? 1u : 0u);
+                    if (m == n_mma - 1) {
+                        // the step is issued: retire its A slot and the B plane that leaves the window
+                        if (leader) tc_commit(&sm.emptyA[sa_slot]);
+#pragma unroll
+                        for (int q = QMAX; q >= 0; --q) {
+                            const int last = HI - q < kPlanes - 1 ? HI - q : kPlanes - 1;
+                            if (last == pa && leader) tc_commit(&sm.emptyB[(cntB + (uint32_t)(QMAX - q)) % kNB3]);
+                        }
+                    }
+                    const int jw = m - (n_mma - n_wait);
+                    if (jw >= 0 && jw < n_wait) next_wait(jw);
+                }
+            }
+            ++cntA;
+        }
+        cntB += QMAX + 1;
+    }
+}
+
+// int32 -> double without the (slow) I2F.F64: the bits 0x43300000'(v + 2^31) are the double 2^52 + 2^31 + v
+__device__ __forceinline__ double i32_to_f64(int32_t v) {
+    return __hiloint2double(0x43300000, (int)((uint32_t)v ^ 0x80000000u)) - 4503601774854144.0;
+}
+
+// epilogue of one pass: this warp's 32 rows x 64 columns
+template <int LO, int HI>
+__device__ __forceinline__ void oz3_epilogue_pass(uint32_t tmem_base, int quad, int half, double* crow, double w_hi) {
+    constexpr int NACC = HI - LO + 1;
+#pragma unroll 1
+    for (int c0 = 64 * half; c0 < 64 * half + 64; c0 += 16) {
+        int32_t v[NACC][16];
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) tmem_ld16(tmem_base + ((uint32_t)(32 * quad) << 16) + (uint32_t)(a * kTileN3 + c0), v[a]);
+        double2 c[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) c[j] = *reinterpret_cast<const double2*>(crow + c0 + 2 * j);
+        tmem_ld_wait();
+        double acc[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) acc[j] = 0.0;
+        double w = w_hi;
+#pragma unroll
+        for (int a = NACC - 1; a >= 0; --a) {                          // smallest weight first
+#pragma unroll
+            for (int j = 0; j < 16; ++j) acc[j] = fma(i32_to_f64(v[a][j]), w, acc[j]);
+            w *= (double)(1 << kDigitBits);
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            c[j].x -= acc[2 * j];
+            c[j].y -= acc[2 * j + 1];
+            *reinterpret_cast<double2*>(crow + c0 + 2 * j) = c[j];
+        }
+    }
+}
+
+// how many k-chunks before the end of a pass its C tile is prefetched into L2 (about 8 us of MMAs: long enough for HBM,
+// short enough that the operand stream does not evict it again)
+__host__ __device__ constexpr int oz3_prefetch_lead(int pass) { return pass == 0 ? 6 : 3; }
+
+// mapA / mapB: boxes of {128 bytes of k, 128 rows, 1 plane}, 128-byte swizzle.  p.kc0 / p.kchunks count 32-byte chunks and
+// must be multiples of 4; p.tiles_n counts 128-column tiles.  PROBE (measurement only, 0 in the product): 1 = the producers
+// skip their TMA loads (the MMAs run on whatever the slots hold), 2 = the issuer skips its MMAs (loads only), 3 = time
+// stamps of one tile of CTA 0 in g_oz3_probe.
+template <int PROBE = 0>
+__global__ void __launch_bounds__(kThreads3, 1)
+ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
     extern __shared__ char smem_raw[];
     char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    uint64_t* full = reinterpret_cast<uint64_t*>(base + kStages2 * kSlotBytes2);
-    uint64_t* empty = full + kStages2;
-    uint64_t* tmem_full = empty + kStages2;
-    uint64_t* tmem_empty = tmem_full + 1;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 1);
+    Oz3Smem sm;
+    sm.slotA = base;
+    sm.slotB = base + kNA3 * kSlotBytes3;
+    sm.fullA = reinterpret_cast<uint64_t*>(base + (kNA3 + kNB3) * kSlotBytes3);
+    sm.emptyA = sm.fullA + kNA3;
+    sm.fullB = sm.emptyA + kNA3;
+    sm.emptyB = sm.fullB + kNB3;
+    sm.tmem_full = sm.emptyB + kNB3;
+    sm.tmem_empty = sm.tmem_full + 1;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sm.tmem_empty + 1);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages2; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-        mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, 4);
+        for (int s = 0; s < kNA3; ++s) { mbar_init(&sm.fullA[s], 1); mbar_init(&sm.emptyA[s], 1); }
+        for (int s = 0; s < kNB3; ++s) { mbar_init(&sm.fullB[s], 1); mbar_init(&sm.emptyB[s], 1); }
+        mbar_init(sm.tmem_full, 1);
+        mbar_init(sm.tmem_empty, 8);
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc(tmem_slot, kTmemCols);
@@ -455,113 +616,97 @@ ozaki_contract_kernel2(const __grid_constant__ OzParams p, const __grid_constant
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     const int ntiles = p.tiles_m * p.tiles_n;
-    constexpr int kPlaneBytes = kTileM * kChunk;                    // 4 KB
-    constexpr int kHalf = 4 * kPlaneBytes;                          // one TMA box: 4 planes
+    const int nchunks = p.kchunks / kKSteps3;
+    const int kbyte0 = p.kc0 * kChunk;
 
-    if (warp == 0) {
-        // ===== TMA producer =====
-        if (lane == 0) {
-            tma_prefetch_desc(&mapA);
-            tma_prefetch_desc(&mapB);
-            int stage = 0, phase = 0;
-            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-                const int tm = tile / p.tiles_n, tn = tile % p.tiles_n;
-                if (!oz_tile<kTileN2>(p, tm, tn).wanted) continue;
-                for (int pass = 0; pass < 2; ++pass)
-                    for (int kc = 0; kc < p.kchunks; ++kc) {
-                        mbar_wait(&empty[stage], (uint32_t)(phase ^ 1));
-                        char* dst = base + (size_t)stage * kSlotBytes2;
-                        const int k = (p.kc0 + kc) * kChunk, ra = p.row0a + tm * kTileM, rb = p.row0b + tn * kTileN2;
-                        mbar_arrive_expect_tx(&full[stage], (uint32_t)(pass ? 4 * kHalf : 2 * kHalf));
-                        tma_load_3d(dst, &mapA, k, ra, 0, &full[stage]);
-                        tma_load_3d(dst + 2 * kHalf, &mapB, k, rb, 0, &full[stage]);
-                        if (pass) {
-                            tma_load_3d(dst + kHalf, &mapA, k, ra, 4, &full[stage]);
-                            tma_load_3d(dst + 3 * kHalf, &mapB, k, rb, 4, &full[stage]);
-                        }
-                        if (++stage == kStages2) { stage = 0; phase ^= 1; }
+    if (warp == 0 || warp == 10) {
+        // ===== producers (whole warps, side effects by one elected lane): warp 0 streams the A planes 0 .. HI of every
+        // (pass, chunk) and prefetches the C tile into L2 shortly before the pass ends, warp 10 the B planes HI .. 0 =====
+        const bool leader = elect_one();
+        const bool isA = warp == 0;
+        const CUtensorMap* map = isA ? &mapA : &mapB;
+        if (leader) tma_prefetch_desc(map);
+        uint64_t* full = isA ? sm.fullA : sm.fullB;
+        uint64_t* empty = isA ? sm.emptyA : sm.emptyB;
+        char* slots = isA ? sm.slotA : sm.slotB;
+        const uint32_t nslots = isA ? kNA3 : kNB3;
+        uint32_t cnt = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int tm = tile / p.tiles_n, tn = tile % p.tiles_n;
+            const OzTile ot = oz_tile<kTileN3>(p, tm, tn);
+            if (!ot.wanted) continue;
+            const int row = isA ? p.row0a + tm * kTileM : p.row0b + tn * kTileN3;
+            for (int pass = 0; pass < 2; ++pass) {
+                const int qmax = oz3_hi(pass);
+                const int pf = nchunks > oz3_prefetch_lead(pass) ? nchunks - oz3_prefetch_lead(pass) : 0;
+                for (int kc = 0; kc < nchunks; ++kc) {
+                    if (isA && kc == pf && PROBE != 1) {
+#pragma unroll
+                        for (int r = 0; r < kTileM; r += 32) l2_prefetch_bulk(ot.c + (size_t)(r + lane) * ot.ld, kTileN3 * (uint32_t)sizeof(double));
                     }
+                    for (int i = 0; i <= qmax; ++i) {
+                        const uint32_t slot = cnt % nslots;
+                        mbar_wait(&empty[slot], ((cnt / nslots) & 1u) ^ 1u);
+                        if (leader) {
+                            if (PROBE == 1) {
+                                mbar_arrive(&full[slot]);
+                            } else {
+                                mbar_arrive_expect_tx(&full[slot], (uint32_t)kSlotBytes3);
+                                tma_load_3d(slots + (size_t)slot * kSlotBytes3, map, kbyte0 + kc * kChunk3, row, isA ? i : qmax - i, &full[slot]);
+                            }
+                        }
+                        ++cnt;
+                    }
+                }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
-            int stage = 0, phase = 0, tphase = 0;
-            for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-                if (!oz_tile<kTileN2>(p, tile / p.tiles_n, tile % p.tiles_n).wanted) continue;
-                for (int pass = 0; pass < 2; ++pass) {
-                    mbar_wait(tmem_empty, (uint32_t)(tphase ^ 1));      // the epilogue has drained the previous four level sums
-                    tc_fence_after();
-                    for (int kc = 0; kc < p.kchunks; ++kc) {
-                        mbar_wait(&full[stage], (uint32_t)phase);
-                        tc_fence_after();
-                        const uint32_t sa = smem_u32(base + (size_t)stage * kSlotBytes2), sb = sa + 2 * kHalf;
-                        const uint32_t acc = (kc > 0) ? 1u : 0u;
-                        if (pass == 0) {
-#pragma unroll
-                            for (int pa = 0; pa < 4; ++pa)
-#pragma unroll
-                                for (int pb = 0; pb + pa < 4; ++pb)
-                                    mma_i8(tmem_base + (uint32_t)((pa + pb) * kTileN2), smem_desc_sw32(sa + pa * kPlaneBytes),
-                                           smem_desc_sw32(sb + pb * kPlaneBytes), kIdescI8N128, pa > 0 ? 1u : acc);
-                        } else {
-#pragma unroll
-                            for (int pa = 0; pa < kPlanes; ++pa)
-#pragma unroll
-                                for (int pb = 0; pb < kPlanes; ++pb)
-                                    if (pa + pb >= 4 && pa + pb < kPlanes)
-                                        mma_i8(tmem_base + (uint32_t)(((pa + pb) & 3) * kTileN2), smem_desc_sw32(sa + pa * kPlaneBytes),
-                                               smem_desc_sw32(sb + pb * kPlaneBytes), kIdescI8N128, pa > 0 ? 1u : acc);
-                        }
-                        tc_commit(&empty[stage]);
-                        if (++stage == kStages2) { stage = 0; phase ^= 1; }
-                    }
-                    tc_commit(tmem_full);
-                    tphase ^= 1;
-                }
-            }
+        // ===== MMA issuer (whole warp; the MMAs and commits by one elected lane) =====
+        const bool leader = elect_one();
+        uint32_t cntA = 0, cntB = 0, tphase = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            if (!oz_tile<kTileN3>(p, tile / p.tiles_n, tile % p.tiles_n).wanted) continue;
+            const bool stamp = PROBE == 3 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && leader;
+            mbar_wait(sm.tmem_empty, tphase ^ 1u);                 // the epilogue has drained the previous level sums
+            tc_fence_after();
+            if (stamp) g_oz3_probe[0] = clock64();
+            oz3_issue_pass<oz3_lo(0), oz3_hi(0), PROBE>(sm, tmem_base, nchunks, cntA, cntB, leader);
+            if (stamp) g_oz3_probe[1] = clock64();
+            if (leader) tc_commit(sm.tmem_full);
+            tphase ^= 1u;
+            mbar_wait(sm.tmem_empty, tphase ^ 1u);
+            tc_fence_after();
+            if (stamp) g_oz3_probe[2] = clock64();
+            oz3_issue_pass<oz3_lo(1), oz3_hi(1), PROBE>(sm, tmem_base, nchunks, cntA, cntB, leader);
+            if (stamp) g_oz3_probe[3] = clock64();
+            if (leader) tc_commit(sm.tmem_full);
+            tphase ^= 1u;
         }
     } else {
-        // ===== epilogue: 4 warps, warp w owns the TMEM lanes 32 (w % 4) .. +31 = rows of the tile =====
-        const int quad = warp & 3;
-        int tphase = 0;
+        // ===== epilogue: warps 2-9; warp w owns the TMEM lanes 32 (w % 4) .. +31 (rows) and 64 of the 128 columns =====
+        const int quad = warp & 3, half = (warp - 2) >> 2;
+        uint32_t tphase = 0;
         const double s2 = p.scale ? (*p.scale) : 1.0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const OzTile ot = oz_tile<kTileN2>(p, tile / p.tiles_n, tile % p.tiles_n);
+            const OzTile ot = oz_tile<kTileN3>(p, tile / p.tiles_n, tile % p.tiles_n);
             if (!ot.wanted) continue;
             double* crow = ot.c + (size_t)(32 * quad + lane) * ot.ld;
+#pragma unroll
             for (int pass = 0; pass < 2; ++pass) {
-                mbar_wait(tmem_full, (uint32_t)tphase);
+                mbar_wait(sm.tmem_full, tphase);
                 tc_fence_after();
-                // weight of the LAST level of this pass (3 or 7): w_last is that of level 7, a level up weighs 128 x more
-                const double wl = p.w_last * s2 * (pass ? 1.0 : 268435456.0);       // 128^4
-#pragma unroll 1
-                for (int c0 = 0; c0 < kTileN2; c0 += 16) {
-                    double acc[16];
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) acc[j] = 0.0;
-                    double w = wl;
-#pragma unroll
-                    for (int l = 3; l >= 0; --l) {                            // smallest weight first
-                        int32_t v[16];
-                        tmem_ld16(tmem_base + ((uint32_t)(32 * quad) << 16) + (uint32_t)(l * kTileN2 + c0), v);
-                        tmem_ld_wait();
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) acc[j] = fma((double)v[j], w, acc[j]);
-                        w *= 128.0;
-                    }
-#pragma unroll
-                    for (int j = 0; j < 16; j += 2) {
-                        double2 c = *reinterpret_cast<double2*>(crow + c0 + j);
-                        c.x -= acc[j];
-                        c.y -= acc[j + 1];
-                        *reinterpret_cast<double2*>(crow + c0 + j) = c;
-                    }
-                }
+                const bool stamp = PROBE == 3 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && warp == 2 && lane == 0;
+                if (stamp) g_oz3_probe[4 + 2 * pass] = clock64();
+                // weight of the last level of the pass: w_last is that of level S - 1, a level up weighs 2^bits more
+                if (pass == 0)
+                    oz3_epilogue_pass<oz3_lo(0), oz3_hi(0)>(tmem_base, quad, half, crow, p.w_last * s2 * (double)(1ull << (kDigitBits * (kPlanes - 1 - oz3_hi(0)))));
+                else
+                    oz3_epilogue_pass<oz3_lo(1), oz3_hi(1)>(tmem_base, quad, half, crow, p.w_last * s2);
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(tmem_empty);
-                tphase ^= 1;
+                if (lane == 0) mbar_arrive(sm.tmem_empty);
+                if (stamp) g_oz3_probe[5 + 2 * pass] = clock64();
+                tphase ^= 1u;
             }
         }
     }

@@ -22,7 +22,8 @@ def gp():
     return binding
 
 
-@pytest.mark.parametrize("m,n", [(128, 32), (256, 512), (640, 1056)])
+# (256, 512), (384, 1152) and (1280, 2048) take the 128 x 128 two-pass kernel, the others the 128 x 64 one (m or n not a multiple of 128)
+@pytest.mark.parametrize("m,n", [(128, 32), (256, 512), (640, 1056), (384, 1152), (1280, 2048)])
 def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
     rng = np.random.default_rng(m + n)
     V = rng.uniform(-0.9, 0.9, size=(n, m))                     # |V| <= 1 as for V = L^-1 K_{X,X^} with v = 1
@@ -39,11 +40,13 @@ def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
     np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
 
 
-def test_planes_are_an_exact_fixed_point_expansion_and_products_are_exact(gp):
+@pytest.mark.parametrize("ma,nb,k", [(256, 192, 288), (384, 256, 640), (128, 128, 128)])
+def test_planes_are_an_exact_fixed_point_expansion_and_products_are_exact(gp, ma, nb, k):
     """x / scale = sum_p d_p 2^(-7 (p+1)) to 2^-57, and the tensor-core result equals the integer arithmetic of the
-    planes recombined in FP64 (levels smallest first), bit for bit up to the last rounding."""
+    planes recombined in FP64 (levels smallest first), bit for bit up to the last roundings (the 128 x 128 kernel, second
+    and third shape, subtracts the levels 0-3 and the levels 4-7 in two steps)."""
     rng = np.random.default_rng(3)
-    ma, nb, k, scale = 256, 192, 288, 4.0
+    scale = 4.0
     A = rng.uniform(-1.9, 1.9, size=(ma, k)); B = rng.normal(size=(nb, k)).clip(-1.9, 1.9)
     dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
     pa, pb = gp.gp_ozaki_slice(dA, scale), gp.gp_ozaki_slice(dB, scale)

@@ -332,7 +332,7 @@ def measure_fp64_peak(gp, torch):
     a.record(); flops = gp.gp_contraction_bench_launch(K, reps, buf); b.record(); torch.cuda.synchronize()
     out["contraction_k1024_tflops"] = flops / (a.elapsed_time(b) * 1e-3) / 1e12
     del buf
-    # the same contraction emulated on the int8 tensor cores (8 digit planes, 36 int8 GEMMs)
+    # the same contraction emulated on the int8 tensor cores (7 planes of 8-bit digits, 28 int8 GEMMs)
     ma = nb = 8192; kk = 4096
     A = torch.rand(ma, kk, dtype=torch.float64, device="cuda") - 0.5
     Ap = gp.gp_ozaki_slice(A, 2.0)
@@ -344,7 +344,8 @@ def measure_fp64_peak(gp, torch):
         if r > 0:
             best = max(best, 2.0 * ma * nb * kk / (a.elapsed_time(b) * 1e-3) / 1e12)
     out["ozaki_int8_contraction_fp64_equivalent_tflops"] = best
-    out["ozaki_int8_pops"] = best * 36 / 1e3
+    S = gp.gp_ozaki_planes()
+    out["ozaki_int8_pops"] = best * (S * (S + 1) // 2) / 1e3
     del A, Ap, C
     return out
 
@@ -530,7 +531,7 @@ def run_b200(args):
         next_rows["cholesky_mixed_int8_emulated"] = {
             "ms": mixed_ms, "gflops_fp64_equivalent": n ** 3 / 3.0 / (mixed_ms * 1e-3) / 1e9, "info": int(pipe.info.item()),
             "rel_diff_to_fp64_factor": float((Lmx - L64).norm() / L64.norm()),
-            "what": "FP64 POTRF/TRSM tile tasks on the executor + SYRK/GEMM tile tasks as 8-plane split-operand int8 products "
+            "what": "FP64 POTRF/TRSM tile tasks on the executor + SYRK/GEMM tile tasks as split-operand int8 products (7 planes of 8-bit digits) "
                     "(tcgen05.mma kind::i8, TMEM accumulators); not the headline: dtype of `value` stays f64"}
         del L64, Lmx, mwork
         pipe.assemble(dX); pipe.cholesky(); pipe.solve(dY)       # leave the FP64 factor behind for what follows

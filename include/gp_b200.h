@@ -203,22 +203,26 @@ int gp_contraction_bench_launch(int K, int reps, void* d_buf, size_t buf_bytes, 
  * hardware capabilities"): the building block of a tensor-core route past the FP64 pipe -- the contraction
  * C -= A B^T in FP64 accuracy EMULATED on the int8 tensor cores (tcgen05.mma kind::i8, int32 accumulators in TMEM)
  * by the split-operand (Ozaki) scheme.  Every operand entry is written in fixed point with one global scale,
- *     x / scale = sum_{p=0}^{7} d_p 2^(-7 (p + 1)),   d_p in [-64, 64]  (8 planes of balanced base-128 digits),
- * the 36 plane products with p + q <= 7 are exact integer GEMMs, and only their recombination rounds (FP64).
- * The truncation is 2^-56 scaleA scaleB per term, below the FP64 rounding of a result of that size.
- *   gp_ozaki_plane_bytes: size of the plane array of a rows x k operand (8 rows k bytes).
- *   gp_ozaki_slice: dX [rows x k] row-major FP64 with leading dimension ld  ->  dPlanes [8][rows][k] int8.
- *        Requires |x| <= scale / 2 for every entry; *d_overflow (device int) is set to 1 otherwise, else 0.
+ *     x / scale = sum_{p=0}^{S-1} d_p 2^(-b (p + 1)),   d_p in [-2^(b-1), 2^(b-1) - 1]   (S planes of balanced b-bit digits;
+ *     S = gp_ozaki_planes() = 7, b = gp_ozaki_digit_bits() = 8: 56 bits of fixed point),
+ * the S (S + 1) / 2 = 28 plane products with p + q <= S - 1 are exact integer GEMMs, and only their recombination rounds
+ * (FP64).  The truncation is 2^-(b (S + 1)) scaleA scaleB per term, below the FP64 rounding of a result of that size.
+ *   gp_ozaki_plane_bytes: size of the plane array of a rows x k operand (S rows k bytes).
+ *   gp_ozaki_slice: dX [rows x k] row-major FP64 with leading dimension ld  ->  dPlanes [S][rows][k] int8.
+ *        Requires |x| <= 0.498 scale for every entry (the top digit must fit); *d_overflow (device int) is set to 1 otherwise, else 0.
  *        k % 32 == 0.
  *   gp_ozaki_contract: dC [ma x nb] row-major FP64, leading dimension ldc (even)  -=  A B^T from the planes of
- *        A [ma x k] and B [nb x k].  ma % 128 == 0, nb % 64 == 0, k % 32 == 0, k <= 65536 (int32 accumulators).
- * Both calls are stream-ordered.  This is a measured building block (bench.py reports its FP64-equivalent rate
- * beside the DMMA contraction); gp_cholesky_tiled does not use it. */
+ *        A [ma x k] and B [nb x k].  ma % 128 == 0, nb % 64 == 0, k % 32 == 0.  An int32 level accumulator takes a
+ *        contraction depth of 16384; deeper contractions run as consecutive launches over k segments.
+ * Both calls are stream-ordered.  bench.py reports the FP64-equivalent rate of the emulated contraction beside the DMMA
+ * contraction; gp_cholesky_tiled does not use it (gp_cholesky_tiled_mixed does). */
+int gp_ozaki_planes(void);
+int gp_ozaki_digit_bits(void);
 int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes);
-/* Output-tile shape of the emulated contraction: 64 (= 0 = auto: 128 x 64 output tile, all eight level sums resident in
- * tensor memory, one pass over k) or 128 (128 x 128 output tile, the levels in two passes of four; needs a column count
- * that is a multiple of 128).  Both were measured at the same 2.3-2.45 int8 POPS (they move the same bytes from L2 to
- * shared memory per product, which is what bounds them); measurement support. */
+/* Output-tile shape of the emulated contraction: 0 = auto (the 128 x 128 two-pass kernel whenever the column count and
+ * the k range are multiples of 128, else the 128 x 64 kernel with all level sums resident in tensor memory), 64 = always
+ * the 128 x 64 kernel, 128 = same as auto.  Measurement support: an MMA of 128 x 64 x 32 takes 48 cycles (shared-memory
+ * operand read), one of 128 x 128 x 32 takes 64, which is the tensor core's full rate. */
 int gp_set_ozaki_tile_n(int n);
 int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double scale, int8_t* dPlanes, int* d_overflow,
                    void* stream);
@@ -232,7 +236,7 @@ int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes
  *   (tile (I,J) -= L(I,0:J) L(J,0:J)^T from the digit planes of the finished columns), then its FP64 panel step runs on
  *   the persistent executor (POTRF tile task + TRSM tile tasks), then its tiles are sliced into digit planes.  The
  *   fixed-point scale is found on the device from max_i K_ii (|L_ij| <= sqrt(K_ii)).  Everything is stream-ordered.
- *   Accuracy: the emulation truncates at 2^-56 of the scale; measured |L - L_oracle| / |L_oracle| ~ 1e-13 (tests).
+ *   Accuracy: the emulation truncates below 2^-56 of the scale; measured |L - L_oracle| / |L_oracle| ~ 1e-13 (tests).
  *   Same arguments and *d_info semantics as gp_cholesky_tiled; additionally tile % 128 == 0, n / tile <= 60, n <= 65536.
  *   dWork: at least gp_mixed_workspace_bytes() (dominated by the dense digit planes, 8 n^2 bytes). */
 int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes);

@@ -25,7 +25,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
-           "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
+           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
            "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n",
@@ -368,6 +368,14 @@ def gp_predict_full_cov_mixed(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor
                                             _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_full_cov_mixed")
 
 
+def gp_ozaki_planes() -> int:
+    return int(load().gp_ozaki_planes())
+
+
+def gp_ozaki_digit_bits() -> int:
+    return int(load().gp_ozaki_digit_bits())
+
+
 def gp_set_ozaki_tile_n(n: int) -> None:
     _check(load().gp_set_ozaki_tile_n(int(n)), "gp_set_ozaki_tile_n")
 
@@ -383,7 +391,7 @@ def gp_ozaki_slice(X: torch.Tensor, scale: float) -> torch.Tensor:
            "gp_ozaki_slice")
     if int(overflow.item()) != 0:
         raise ValueError("gp_ozaki_slice: an entry exceeds scale / 2")
-    return planes.view(8, rows, k)
+    return planes.view(int(load().gp_ozaki_planes()), rows, k)
 
 
 def gp_ozaki_contract(Aplanes: torch.Tensor, Bplanes: torch.Tensor, scaleA: float, scaleB: float, C: torch.Tensor) -> None:

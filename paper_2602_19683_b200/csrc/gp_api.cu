@@ -869,7 +869,9 @@ namespace {
 std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (128 when the shape allows), 64, 128: gp_set_ozaki_tile_n (measurement support)
 
 // launches the emulated contraction described by q (kc0 / kchunks in 32-byte chunks) with the tile shape that fits:
-// the 128 x 128 two-pass kernel when the column count and the k range are multiples of 128, else the 128 x 64 one
+// the 128 x 128 two-pass kernel when the column count and the k range are multiples of 128, else the 128 x 64 one.
+// A contraction deeper than oz::kMaxK (the depth an int32 level accumulator can take) runs as several launches over
+// consecutive k segments, each subtracting its part from C.
 int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const int8_t* planesB, uint64_t rowsB, uint64_t kdim, int64_t ncols,
                  cudaStream_t st) {
     const int want = g_ozaki_tile_n.load(std::memory_order_relaxed);
@@ -882,20 +884,26 @@ int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const in
         rc = configure_once(1024u, [] {
             return cudaFuncSetAttribute(oz::ozaki_contract_kernel3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz3) == cudaSuccess;
         });
-        if (rc != GP_OK) return rc;
         q.tiles_n = (int)(ncols / oz::kTileN3);
-        const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
-        oz::ozaki_contract_kernel3<0><<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB);
     } else {
         if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM)) != GP_OK) return rc;
         if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN)) != GP_OK) return rc;
         rc = configure_once(512u, [] {
             return cudaFuncSetAttribute(oz::ozaki_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz) == cudaSuccess;
         });
-        if (rc != GP_OK) return rc;
         q.tiles_n = (int)(ncols / oz::kTileN);
-        const int64_t tiles = (int64_t)q.tiles_m * q.tiles_n;
-        oz::ozaki_contract_kernel<<<(int)std::min<int64_t>(tiles, sm_count()), oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
+    }
+    if (rc != GP_OK) return rc;
+    const int grid = (int)std::min<int64_t>((int64_t)q.tiles_m * q.tiles_n, sm_count());
+    const int seg_chunks = oz::kMaxK / oz::kChunk;                      // a multiple of 4
+    const int first = q.kc0, total = q.kchunks;
+    for (int done = 0; done < total; done += seg_chunks) {
+        q.kc0 = first + done;
+        q.kchunks = std::min(seg_chunks, total - done);
+        if (wide)
+            oz::ozaki_contract_kernel3<0><<<grid, oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB);
+        else
+            oz::ozaki_contract_kernel<<<grid, oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
     }
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
@@ -906,6 +914,9 @@ extern "C" int gp_set_ozaki_tile_n(int n) {
     g_ozaki_tile_n.store(n, std::memory_order_relaxed);
     return GP_OK;
 }
+
+extern "C" int gp_ozaki_planes(void) { return oz::kPlanes; }
+extern "C" int gp_ozaki_digit_bits(void) { return oz::kDigitBits; }
 
 extern "C" int gp_ozaki_plane_bytes(int64_t rows, int64_t k, size_t* bytes) {
     if (!bytes) return GP_ERR_NULL;
@@ -930,8 +941,7 @@ extern "C" int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t
 extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,
                                  double scaleB, double* dC, int64_t ldc, void* stream) {
     if (!dAplanes || !dBplanes || !dC) return GP_ERR_NULL;
-    // int32 accumulators: at most S pairs of |d| <= 64 digits per level and k-step: 8 * 2^12 * k < 2^31
-    if (ma <= 0 || nb <= 0 || k <= 0 || ma % oz::kTileM != 0 || nb % oz::kTileN != 0 || k % oz::kChunk != 0 || k > 65536 || ldc < nb || ldc % 2 != 0)
+    if (ma <= 0 || nb <= 0 || k <= 0 || ma % oz::kTileM != 0 || nb % oz::kTileN != 0 || k % oz::kChunk != 0 || k > (1 << 22) || ldc < nb || ldc % 2 != 0)
         return GP_ERR_SIZE;
     if (!(scaleA > 0.0) || !(scaleB > 0.0) || !std::isfinite(scaleA * scaleB)) return GP_ERR_HYPER;
     oz::OzParams p;
@@ -964,7 +974,7 @@ int mixed_ok(int64_t n, int tile) {
     if (rc != GP_OK) return rc;
     if (tile % 128 != 0) return GP_ERR_TILE;
     if (n / tile > 60) return GP_ERR_SIZE;                 // one ticket counter per panel launch in the 256-byte header
-    if (n > 65536 + 128) return GP_ERR_SIZE;               // int32 accumulators of the emulated contraction: k <= 65536
+    if (n > 65536 + 128) return GP_ERR_SIZE;               // 8.6 GB of digit planes per 32768^2 entries: the workspace is the limit
     return GP_OK;
 }
 }  // namespace
@@ -1053,7 +1063,7 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     q.t = tile;
     q.J = J;
     q.row0a = q.row0b = J * tile;
-    // both operands come from the dense digit planes [8][n][n] of the whole matrix
+    // both operands come from the dense digit planes [S][n][n] of the whole matrix
     return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, c.st);
 }
 
@@ -1180,7 +1190,7 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
     }
     if ((rc = launch_trtri_any(b, dL, tile, NB, invD, st)) != GP_OK) return rc;
     // fixed-point scales: |L_ij| <= max |L| (read from the factor), |V_ia| <= sqrt(k(x^_a, x^_a)) = sqrt(v)
-    const double sv = std::ldexp(1.0, (int)std::ceil(std::log2(std::sqrt(h.vertical))) + 1);
+    const double sv = std::ldexp(1.0, (int)std::ceil(std::log2(std::sqrt(h.vertical) / 0.98)) + 1);   // |V_ia| <= sqrt(v) <= 0.49 sv
     const int64_t lcount = (int64_t)M * (M + 1) / 2 * tile * tile;
     oz::absmax_lower_tiles_kernel<<<sm_count() * 8, 256, 0, st>>>(dL, lcount, maxbits);
     oz::finish_scales_kernel<<<1, 1, 0, st>>>(maxbits, sv, scale);

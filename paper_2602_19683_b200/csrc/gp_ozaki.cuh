@@ -4,27 +4,27 @@
 // sm_100a has no FP64 kind of tcgen05.mma, and the FP64 DMMA path of gp_gemm.cuh already runs at 93 % of the
 // chip's FP64 rate.  The only way to a materially faster  C -= A B^T  in FP64 accuracy is to EMULATE it on the
 // integer tensor cores (the Ozaki scheme): write every operand entry in fixed point with one global scale,
-//     x / scale = sum_{p=0}^{S-1} d_p 2^{-7 (p+1)},      d_p in [-64, 64]   (balanced base-128 digits, int8),
+//     x / scale = sum_{p=0}^{S-1} d_p 2^{-b (p+1)},      d_p in [-2^(b-1), 2^(b-1) - 1]   (balanced digits, int8),
 // so that
-//     A B^T = scaleA scaleB sum_{lvl} 2^{-7 (lvl + 2)} sum_{p+q = lvl} D_p(A) D_q(B)^T .
-// Every digit-plane product is an int8 GEMM whose int32 accumulation is EXACT (|d| <= 64: 2^12 per term, so
-// 2^19 terms fit), products of equal weight share one accumulator, and only the final recombination of the S
-// level sums rounds (in FP64).  Pairs with p + q >= S are dropped: with S = 8 that is 2^-56 relative to
-// scaleA scaleB, below the FP64 rounding of the result.  Measured on the CPU (a tiled Cholesky whose trailing
-// updates are emulated this way, cond(K) = 4e4): S = 6 / 7 / 8 planes give |L - L_fp64| / |L| =
-// 1.7e-9 / 1.4e-11 / 1.2e-13, so S = 8 (36 int8 GEMMs per FP64 GEMM) is what north_star's 1e-10 needs with margin.
+//     A B^T = scaleA scaleB sum_{lvl} 2^{-b (lvl + 2)} sum_{p+q = lvl} D_p(A) D_q(B)^T .
+// Every digit-plane product is an int8 GEMM whose int32 accumulation is EXACT, products of equal weight share one
+// accumulator, and only the final recombination of the S level sums rounds (in FP64).  Pairs with p + q >= S are
+// dropped: that is 2^-(b (S + 1)) relative to scaleA scaleB per term, below the FP64 rounding of the result.
+// S = 7 planes of b = 8 bits (56 bits of fixed point, S (S + 1) / 2 = 28 int8 GEMMs per FP64 GEMM).  Round 2 began with
+// 8 planes of 7 bits (36 GEMMs; a CPU study of the tiled Cholesky with emulated updates at cond(K) = 4e4 gave
+// |L - L_fp64| / |L| = 1.7e-9 / 1.4e-11 / 1.2e-13 for 42 / 49 / 56 bits, so 56 bits is what north_star's 1e-10 needs
+// with margin); the 8-bit digits keep the 56 bits with 22 % fewer MMAs, which counts double because the kernel
+// runs into the board's POWER limit on real operands (profiles/r02_ozaki_bounds.md).  The price is the depth one
+// accumulator can take: 7 * 2^14 * k < 2^31 means k <= 16384 (kMaxK), longer contractions run in segments.
+// The digits are balanced (round to nearest), not the bytes of the two's complement: unsigned low digits would
+// turn the dropped terms into a bias instead of zero-mean noise.
 //
-// Kernel (this IS Blackwell-native: tcgen05.mma kind::i8, accumulators in TMEM, operands by TMA):
-//   * output tile 128 x 64 per CTA; the S = 8 level accumulators (int32) fill the SM's tensor memory exactly:
-//     8 x 64 = 512 columns x 128 lanes;
-//   * a stage holds one 32-deep k-chunk of ALL planes of both operands (8 x 128 x 32 B + 8 x 64 x 32 B = 48 KB,
-//     two 3-D TMA loads with the 32-byte swizzle), so every operand byte is fetched once and used by all the
-//     pairs it takes part in: 36 MMAs (128 x 64 x 32) per stage, ring of 4 stages;
-//   * warp 0 = TMA producer, warp 1 = MMA issuer (one elected lane; tcgen05.commit releases stages and hands the
-//     finished tile over), warps 2-5 = epilogue: tcgen05.ld the eight level sums of a row segment, convert,
-//     recombine smallest weight first in FP64, C -= result.
-// Status: a measured building block with its own entry points and parity test; the executor still runs the FP64
-// DMMA path (DESIGN.md section 10 says what the measurement implies).
+// Kernels (Blackwell-native: tcgen05.mma kind::i8, accumulators in TMEM, operands by TMA):
+//   * ozaki_contract_kernel3 (the default): 128 x 128 output tile, levels in two passes -- see its own comment;
+//   * ozaki_contract_kernel: 128 x 64 output tile for shapes that are not multiples of 128; all S level accumulators
+//     in tensor memory at once (7 x 64 columns); a stage holds one 32-deep k-chunk of ALL planes of both operands
+//     (two 3-D TMA loads with the 32-byte swizzle), ring of 4 stages; warp 0 = TMA producer, warp 1 = MMA issuer,
+//     warps 2-5 = epilogue (tcgen05.ld the level sums of a row segment, recombine smallest weight first, C -= result).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -35,8 +35,12 @@
 namespace gpb {
 namespace oz {
 
-constexpr int kPlanes = 8;           // S
-constexpr int kDigitBits = 7;
+constexpr int kPlanes = 7;           // S
+constexpr int kDigitBits = 8;        // balanced base-256 digits in [-128, 127]: S * bits = 56 bits of fixed point
+constexpr int kFixedBits = kPlanes * kDigitBits;
+constexpr long long kDigitHalf = 1ll << (kDigitBits - 1), kDigitMask = (1ll << kDigitBits) - 1;
+// int32 accumulators: a level sums at most S products of two digits per k-step, S * 2^(2 (bits - 1)) * k < 2^31
+constexpr int kMaxK = 16384;         // 7 * 2^14 * 16384 = 1.88e9 < 2^31; longer contractions are run in segments
 constexpr int kTileM = 128, kTileN = 64, kChunk = 32;
 constexpr int kStagesOz = 4;
 constexpr int kABytes = kPlanes * kTileM * kChunk;       // 32 KB
@@ -47,7 +51,7 @@ constexpr int kSmemOz = kStagesOz * kStageBytesOz + 1024 + 256;
 constexpr int kTmemCols = 512;
 
 // ---- slicing: FP64 -> S planes of balanced base-128 digits ------------------------------------------------------
-// planes[p][r][k] (int8, row-major rows x k per plane).  |x| <= scale / 2 is required (the top digit must fit).
+// planes[p][r][k] (int8, row-major rows x k per plane).  |x| <= 0.498 scale is required (the top digit must stay <= 127).
 __global__ void __launch_bounds__(256) slice_kernel(const double* __restrict__ X, int64_t rows, int64_t k, int64_t ld, double inv_scale,
                                                     int8_t* __restrict__ planes, int* __restrict__ overflow) {
     const int64_t total = rows * (k / 4);
@@ -59,10 +63,10 @@ __global__ void __launch_bounds__(256) slice_kernel(const double* __restrict__ X
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const double x = X[r * ld + c + e] * inv_scale;                       // |x| <= 1/2
-            long long I = __double2ll_rn(x * 72057594037927936.0);                  // 2^56 = 2^(7 S)
+            long long I = __double2ll_rn(x * (double)(1ull << kFixedBits));
 #pragma unroll
             for (int p = kPlanes - 1; p >= 0; --p) {
-                const long long d = ((I + 64) & 127) - 64;
+                const long long d = ((I + kDigitHalf) & kDigitMask) - kDigitHalf;
                 I = (I - d) >> kDigitBits;
                 packed[p] |= (uint32_t)((int)d & 0xff) << (8 * e);
             }
@@ -93,10 +97,10 @@ __global__ void __launch_bounds__(256) slice_tile_column_kernel(const double* __
         for (int p = 0; p < kPlanes; ++p) packed[p] = 0u;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            long long I56 = __double2ll_rn(xs[e] * inv_scale * 72057594037927936.0);
+            long long I56 = __double2ll_rn(xs[e] * inv_scale * (double)(1ull << kFixedBits));
 #pragma unroll
             for (int p = kPlanes - 1; p >= 0; --p) {
-                const long long d = ((I56 + 64) & 127) - 64;
+                const long long d = ((I56 + kDigitHalf) & kDigitMask) - kDigitHalf;
                 I56 = (I56 - d) >> kDigitBits;
                 packed[p] |= (uint32_t)((int)d & 0xff) << (8 * e);
             }
@@ -124,7 +128,7 @@ __global__ void __launch_bounds__(1024) factor_scale_kernel(const double* __rest
         for (int k = 0; k < 32; ++k) m = fmax(m, s_max[k]);
         int e;
         const double f = frexp(sqrt(m > 0.0 ? m : 1.0), &e);      // sqrt(m) = f 2^e, f in [0.5, 1)
-        const double sc = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0)); // >= 2 sqrt(m), with a little head-room at the edge
+        const double sc = ldexp(1.0, e + 1 + (f > 0.98 ? 1 : 0)); // >= 2 sqrt(m) / 0.98: the top digit of a balanced expansion stays below 2^(b-1)
         scale[0] = sc;
         scale[1] = sc * sc;                                          // the weight factor of a product of two such operands
     }
@@ -144,7 +148,7 @@ __global__ void finish_scales_kernel(const unsigned long long* __restrict__ bits
     const double m = __longlong_as_double((long long)*bits);
     int e;
     const double f = frexp(m > 0.0 ? m : 1.0, &e);
-    const double sl = ldexp(1.0, e + 1 + (f > 0.999 ? 1 : 0));
+    const double sl = ldexp(1.0, e + 1 + (f > 0.98 ? 1 : 0));
     scale[0] = sl;
     scale[1] = sv;
     scale[2] = sl * sv;
@@ -169,10 +173,10 @@ __global__ void __launch_bounds__(256) slice_general_column_kernel(const double*
         for (int p = 0; p < kPlanes; ++p) packed[p] = 0u;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            long long I56 = __double2ll_rn(xs[e] * inv_scale * 72057594037927936.0);
+            long long I56 = __double2ll_rn(xs[e] * inv_scale * (double)(1ull << kFixedBits));
 #pragma unroll
             for (int p = kPlanes - 1; p >= 0; --p) {
-                const long long d = ((I56 + 64) & 127) - 64;
+                const long long d = ((I56 + kDigitHalf) & kDigitMask) - kDigitHalf;
                 I56 = (I56 - d) >> kDigitBits;
                 packed[p] |= (uint32_t)((int)d & 0xff) << (8 * e);
             }
@@ -399,7 +403,7 @@ ozaki_contract_kernel(const __grid_constant__ OzParams p, const __grid_constant_
                     tmem_ld_wait();
 #pragma unroll
                     for (int j = 0; j < 16; ++j) acc[j] = fma((double)v[j], w, acc[j]);
-                    w *= 128.0;
+                    w *= (double)(1 << kDigitBits);
                 }
 #pragma unroll
                 for (int j = 0; j < 16; j += 2) {

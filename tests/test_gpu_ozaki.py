@@ -32,7 +32,8 @@ def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
     A = torch.from_numpy(np.ascontiguousarray(V.T)).cuda()      # m x n, contraction index contiguous
     C = torch.from_numpy(Kss.copy()).cuda()
     planes = gp.gp_ozaki_slice(A, 2.0)
-    assert planes.shape == (8, m, n) and int(planes.min()) >= -64 and int(planes.max()) <= 64
+    S, b = gp.gp_ozaki_planes(), gp.gp_ozaki_digit_bits()
+    assert S * b == 56 and planes.shape == (S, m, n) and int(planes.min()) >= -2 ** (b - 1) and int(planes.max()) <= 2 ** (b - 1) - 1
     gp.gp_ozaki_contract(planes, planes, 2.0, 2.0, C)
     torch.cuda.synchronize()
     got = C.cpu().numpy()
@@ -42,27 +43,46 @@ def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
 
 @pytest.mark.parametrize("ma,nb,k", [(256, 192, 288), (384, 256, 640), (128, 128, 128)])
 def test_planes_are_an_exact_fixed_point_expansion_and_products_are_exact(gp, ma, nb, k):
-    """x / scale = sum_p d_p 2^(-7 (p+1)) to 2^-57, and the tensor-core result equals the integer arithmetic of the
-    planes recombined in FP64 (levels smallest first), bit for bit up to the last roundings (the 128 x 128 kernel, second
-    and third shape, subtracts the levels 0-3 and the levels 4-7 in two steps)."""
+    """x / scale = sum_p d_p 2^(-b (p+1)) to 2^-57 (S planes of b-bit digits, S b = 56), and the tensor-core result equals
+    the integer arithmetic of the planes recombined in FP64 (levels smallest first), bit for bit up to the last roundings
+    (the 128 x 128 kernel, second and third shape, subtracts the high and the low levels in two steps)."""
     rng = np.random.default_rng(3)
     scale = 4.0
     A = rng.uniform(-1.9, 1.9, size=(ma, k)); B = rng.normal(size=(nb, k)).clip(-1.9, 1.9)
     dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
     pa, pb = gp.gp_ozaki_slice(dA, scale), gp.gp_ozaki_slice(dB, scale)
     Pa, Pb = pa.cpu().numpy().astype(np.int64), pb.cpu().numpy().astype(np.int64)
-    w = 2.0 ** (-7.0 * np.arange(1, 9))
+    S, b = gp.gp_ozaki_planes(), gp.gp_ozaki_digit_bits()
+    w = 2.0 ** (-float(b) * np.arange(1, S + 1))
     np.testing.assert_allclose(np.tensordot(w, Pa.astype(np.float64), axes=1) * scale, A, rtol=0, atol=scale * 2.0 ** -57)
     C0 = rng.normal(size=(ma, nb))
     C = torch.from_numpy(C0.copy()).cuda()
     gp.gp_ozaki_contract(pa, pb, scale, scale, C)
     torch.cuda.synchronize()
     acc = np.zeros((ma, nb))
-    for lvl in range(7, -1, -1):
+    for lvl in range(S - 1, -1, -1):
         s = sum(Pa[p] @ Pb[lvl - p].T for p in range(lvl + 1))          # exact int64
-        acc += s.astype(np.float64) * (scale * scale * 2.0 ** (-7.0 * (lvl + 2)))
+        acc += s.astype(np.float64) * (scale * scale * 2.0 ** (-float(b) * (lvl + 2)))
     np.testing.assert_allclose(C.cpu().numpy(), C0 - acc, rtol=0, atol=4e-16 * np.abs(C0 - acc).max())
     assert relerr(C.cpu().numpy(), C0 - A @ B.T) <= 1e-14
+
+
+def test_contraction_deeper_than_one_accumulator_runs_in_segments(gp):
+    """k = 20480 > 16384 (what an int32 level accumulator takes with 8-bit digits): two launches over k segments.  Operands
+    near +- 0.495 scale with equal signs drive the level sums as high as they go; the expected value is exact rational
+    arithmetic (a floating-point sum of 20480 terms would be the less accurate side)."""
+    from fractions import Fraction
+    m, k, val = 128, 20480, 0.99
+    A = torch.full((m, k), val, dtype=torch.float64, device="cuda")
+    A[::2] = -val
+    C = torch.zeros(m, m, dtype=torch.float64, device="cuda")
+    planes = gp.gp_ozaki_slice(A, 2.0)
+    gp.gp_ozaki_contract(planes, planes, 2.0, 2.0, C)
+    torch.cuda.synchronize()
+    mag = float(Fraction(val) ** 2 * k)
+    sign = np.where(np.arange(m) % 2 == 0, -1.0, 1.0)
+    want = -mag * np.outer(sign, sign)
+    assert relerr(C.cpu().numpy(), want) <= 1e-15
 
 
 def test_slice_reports_entries_beyond_the_scale_and_bad_arguments(gp):

@@ -175,7 +175,7 @@ def test_panel_schedules_of_the_mixed_factorisation_replay(gp, n, tile):
         want = nbt + nbt * (nbt - 1) // 2 + sum((nbt - kk) for jj in range(nbt) for kk in range(jj + 1, nbt)) + (M - J - 1) * nbt
         assert items == want, (J, items, want)
     assert gp.gp_panel_schedule_selfcheck(n, tile, M) == gp.ERR["SIZE"]
-    assert gp.gp_mixed_workspace_bytes(n, tile) >= 8 * n * n
+    assert gp.gp_mixed_workspace_bytes(n, tile) >= gp.gp_ozaki_planes() * n * n
     with pytest.raises(gp.GpError):
         gp.gp_mixed_workspace_bytes(n, 96)
 

@@ -872,15 +872,28 @@ std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (128 when the shape allows
 // the 128 x 128 two-pass kernel when the column count and the k range are multiples of 128, else the 128 x 64 one.
 // A contraction deeper than oz::kMaxK (the depth an int32 level accumulator can take) runs as several launches over
 // consecutive k segments, each subtracting its part from C.
+// c_rows: rows of the 2-D view [c_rows][ld] of the output array (dense: the rows of C, ld = ldc; tiled: tiles x t, ld = t)
 int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const int8_t* planesB, uint64_t rowsB, uint64_t kdim, int64_t ncols,
-                 cudaStream_t st) {
+                 uint64_t c_rows, cudaStream_t st) {
     const int want = g_ozaki_tile_n.load(std::memory_order_relaxed);
     const bool wide = want != 64 && ncols % oz::kTileN3 == 0 && q.kchunks % oz::kKSteps3 == 0 && q.kc0 % oz::kKSteps3 == 0 && kdim % oz::kChunk3 == 0;
-    CUtensorMap mapA, mapB;
+    CUtensorMap mapA, mapB, mapC;
     int rc;
     if (wide) {
         if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM, 1, oz::kChunk3)) != GP_OK) return rc;
         if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN3, 1, oz::kChunk3)) != GP_OK) return rc;
+        {
+            EncodeTiledFn enc = encode_tiled();
+            if (!enc) return GP_ERR_CUDA;
+            const uint64_t ld = (q.tiled == 1 || q.tiled == 2) ? (uint64_t)q.t : (uint64_t)q.ldc;
+            const cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)c_rows};
+            const cuuint64_t strides[1] = {(cuuint64_t)(ld * sizeof(double))};
+            const cuuint32_t box[2] = {(cuuint32_t)oz::kStageCols3, 32};
+            const cuuint32_t estr[2] = {1, 1};
+            if (enc(&mapC, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, q.C, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                return GP_ERR_CUDA;
+        }
         rc = configure_once(1024u, [] {
             return cudaFuncSetAttribute(oz::ozaki_contract_kernel3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz3) == cudaSuccess;
         });
@@ -901,7 +914,7 @@ int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const in
         q.kc0 = first + done;
         q.kchunks = std::min(seg_chunks, total - done);
         if (wide)
-            oz::ozaki_contract_kernel3<0><<<grid, oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB);
+            oz::ozaki_contract_kernel3<0><<<grid, oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB, mapC);
         else
             oz::ozaki_contract_kernel<<<grid, oz::kThreadsOz, oz::kSmemOz, st>>>(q, mapA, mapB);
     }
@@ -951,7 +964,7 @@ extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_
     p.tiles_m = (int)(ma / oz::kTileM);
     p.kchunks = (int)(k / oz::kChunk);
     p.w_last = scaleA * scaleB * std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
-    return launch_ozaki(p, dAplanes, (uint64_t)ma, dBplanes, (uint64_t)nb, (uint64_t)k, nb, (cudaStream_t)stream);
+    return launch_ozaki(p, dAplanes, (uint64_t)ma, dBplanes, (uint64_t)nb, (uint64_t)k, nb, (uint64_t)ma, (cudaStream_t)stream);
 }
 
 // ---- gp_cholesky_tiled_mixed: FP64 panels + emulated trailing updates ------------------------
@@ -1064,7 +1077,7 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     q.J = J;
     q.row0a = q.row0b = J * tile;
     // both operands come from the dense digit planes [S][n][n] of the whole matrix
-    return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, c.st);
+    return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, (uint64_t)c.M * (c.M + 1) / 2 * (uint64_t)tile, c.st);
 }
 
 extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
@@ -1235,7 +1248,7 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
             q.Mt = M;
             q.row0a = 0;
             q.row0b = P * tile;
-            if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesL, (uint64_t)n, (uint64_t)n, tile, st)) != GP_OK) return rc;
+            if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesL, (uint64_t)n, (uint64_t)n, tile, (uint64_t)m * (uint64_t)M, st)) != GP_OK) return rc;
         }
         // the FP64 half of step P: V^T(:, P) <- V^T(:, P) L(P,P)^-T, one ROW_V chain per block row, on the executor
         oz::set_general_column_versions_kernel<<<(NBm * nbt + 255) / 256, 256, 0, st>>>(p.verV, NBm, NB, nbt, P, kConsumerWarps);
@@ -1259,7 +1272,7 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
         q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
         q.scale = scale + 3;
         q.tiled = 3;
-        if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesV, (uint64_t)m, (uint64_t)n, m, st)) != GP_OK) return rc;
+        if ((rc = launch_ozaki(q, planesV, (uint64_t)m, planesV, (uint64_t)m, (uint64_t)n, m, (uint64_t)m, st)) != GP_OK) return rc;
     }
     dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
     mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);

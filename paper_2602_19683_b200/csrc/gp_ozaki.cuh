@@ -282,6 +282,9 @@ struct OzTile {
     bool wanted;
     double* c;            // address of element (row 0 of the tile, column 0 of the tile)
     int64_t ld;
+    // the same place in the 2-D view [rows][ld] of the output array (dense: the matrix itself; tiled: tile after tile, each
+    // t rows of t entries) that the wide kernel's tensor map for C describes
+    int row0, col0;
 };
 template <int TN = kTileN>
 __device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
@@ -289,7 +292,9 @@ __device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
     if (p.tiled == 0 || p.tiled == 3) {
         o.wanted = p.tiled == 0 || tn * TN < (tm + 1) * kTileM;
         o.ld = p.ldc;
-        o.c = p.C + (size_t)tm * kTileM * p.ldc + (size_t)tn * TN;
+        o.row0 = tm * kTileM;
+        o.col0 = tn * TN;
+        o.c = p.C + (size_t)o.row0 * p.ldc + (size_t)o.col0;
         return o;
     }
     const int bpt = p.t / kTileM;                       // 128-row blocks per tile edge
@@ -297,14 +302,18 @@ __device__ __forceinline__ OzTile oz_tile(const OzParams& p, int tm, int tn) {
         const int a = tm / bpt, rblk = tm % bpt;
         o.wanted = true;
         o.ld = p.t;
-        o.c = p.C + ((size_t)a * p.Mt + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * TN;
+        o.row0 = (a * p.Mt + p.J) * p.t + rblk * kTileM;
+        o.col0 = tn * TN;
+        o.c = p.C + (size_t)o.row0 * p.t + (size_t)o.col0;
         return o;
     }
     const int I = p.J + tm / bpt, rblk = tm % bpt;
     // on the diagonal tile only the lower part is data: skip 128 x TN pieces that lie wholly above the diagonal
     o.wanted = !(I == p.J && tn * TN >= (rblk + 1) * kTileM);
     o.ld = p.t;
-    o.c = p.C + ((size_t)I * (I + 1) / 2 + p.J) * (size_t)p.t * p.t + (size_t)rblk * kTileM * p.t + (size_t)tn * TN;
+    o.row0 = (I * (I + 1) / 2 + p.J) * p.t + rblk * kTileM;
+    o.col0 = tn * TN;
+    o.c = p.C + (size_t)o.row0 * p.t + (size_t)o.col0;
     return o;
 }
 
@@ -451,7 +460,7 @@ constexpr int kKSteps3 = kChunk3 / kChunk;                      // MMAs (K = 32)
 constexpr int kSlotBytes3 = kTileM * kChunk3;                   // 16 KB
 constexpr int kNA3 = 5, kNB3 = 8;
 constexpr int kThreads3 = 352;                                  // warp 0 A producer, 1 MMA issuer, 2-9 epilogue, 10 B producer
-constexpr int kSmemOz3 = (kNA3 + kNB3) * kSlotBytes3 + 1024 + 512;
+constexpr int kSmemOz3 = (kNA3 + kNB3) * kSlotBytes3 + 16384 + 1024 + 512;   // slots, epilogue staging, alignment slack, barriers
 constexpr uint32_t kIdescI8N128 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTileN3 >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 
 // the level range of a pass
@@ -474,31 +483,53 @@ struct Oz3Smem {
     uint64_t *fullA, *emptyA, *fullB, *emptyB, *tmem_full, *tmem_empty;
 };
 
+// the same instructions under a predicate instead of a C++ branch: a branch around every MMA splits the issue loop into
+// basic blocks and ptxas then rebuilds the descriptors (R2UR and a dozen uniform ops) between the waits and the first MMA
+// of each step, which is exactly where the tensor core's two-deep queue runs dry
+__device__ __forceinline__ void mma_i8_n128_if(uint32_t leader, uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        " .reg .pred p, q;\n"
+        " setp.ne.b32 p, %4, 0;\n"
+        " setp.ne.b32 q, %6, 0;\n"
+        " @q tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n"
+        "}\n" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(kIdescI8N128), "r"(accumulate), "r"(0u), "r"(leader)
+        : "memory");
+}
+__device__ __forceinline__ void tc_commit_if(uint32_t leader, uint64_t* bar) {
+    asm volatile("{\n .reg .pred q;\n setp.ne.b32 q, %1, 0;\n @q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n}\n" ::"r"(smem_u32(bar)),
+                 "r"(leader)
+                 : "memory");
+}
+
 // issuer: one pass over the k range for one tile.  The tensor core's instruction queue is about two MMAs deep (a pause
 // of more than ~100 cycles in the issuing thread is a bubble in the pipe: profiles/r02_ozaki_bounds.md), so the
-// mbarrier waits of the NEXT step are interleaved with the last MMAs of the current one, and a step's descriptors
-// are one add away from two per-ring base words.
+// mbarrier waits of the NEXT step are interleaved with the last MMAs of the current one, ring positions advance
+// without divisions, and a step's descriptors are one add away from words computed a step ahead.
 template <int LO, int HI, int PROBE>
-__device__ __forceinline__ void oz3_issue_pass(const Oz3Smem& sm, uint32_t tmem_base, int nchunks, uint32_t& cntA, uint32_t& cntB, bool leader) {
+__device__ __forceinline__ void oz3_issue_pass(const Oz3Smem& sm, uint32_t tmem_base, int nchunks, uint32_t& cntA, uint32_t& cntB, uint32_t leader) {
     constexpr int QMAX = HI < kPlanes - 1 ? HI : kPlanes - 1;       // B planes QMAX .. 0 and A planes 0 .. QMAX take part
     constexpr uint64_t kDescHi = ((uint64_t)(1024 >> 4) | ((uint64_t)1 << 14) | ((uint64_t)2 << 29)) << 32;   // SBO, version, SWIZZLE_128B
+    constexpr uint32_t kSlotLo = (uint32_t)(kSlotBytes3 >> 4);
+    static_assert((kNB3 & (kNB3 - 1)) == 0, "the B ring is indexed with a mask");
     const uint32_t a_lo0 = ((smem_u32(sm.slotA) >> 4) & 0x3fffu) | (1u << 16);
     const uint32_t b_lo0 = ((smem_u32(sm.slotB) >> 4) & 0x3fffu) | (1u << 16);
-    // B planes first used by step 0 of a chunk, and the A plane of a step
-    auto wait_b = [&](uint32_t cb, int q) { const uint32_t c = cb + (uint32_t)(QMAX - q); mbar_wait(&sm.fullB[c % kNB3], (c / kNB3) & 1u); };
-    auto wait_a = [&](uint32_t ca) { mbar_wait(&sm.fullA[ca % kNA3], (ca / kNA3) & 1u); };
+    auto wait_b = [&](uint32_t cb, int q) { const uint32_t c = cb + (uint32_t)(QMAX - q); mbar_wait(&sm.fullB[c & (kNB3 - 1)], (c / kNB3) & 1u); };
+    // ring position of the A plane of the current step, and of the next one
+    uint32_t sa = cntA % kNA3, pha = (cntA / kNA3) & 1u;
     // prologue: the operands of step 0 of chunk 0
 #pragma unroll
     for (int q = QMAX; q >= 0; --q)
         if (LO - q <= 0) wait_b(cntB, q);
-    wait_a(cntA);
+    mbar_wait(&sm.fullA[sa], pha);
     for (int kc = 0; kc < nchunks; ++kc) {
         const bool more = kc + 1 < nchunks;
 #pragma unroll
         for (int pa = 0; pa <= QMAX; ++pa) {
-            tc_fence_after();
-            const uint32_t sa_slot = cntA % kNA3;
-            const uint32_t a_lo = a_lo0 + sa_slot * (uint32_t)(kSlotBytes3 >> 4);
+            const uint32_t san = sa + 1 == kNA3 ? 0u : sa + 1, phan = sa + 1 == kNA3 ? pha ^ 1u : pha;
+            const uint32_t a_lo = a_lo0 + sa * kSlotLo;
+            if (PROBE != 6) tc_fence_after();
             // this step's MMAs: pb in [max(0, LO - pa), min(S - 1, HI - pa)], 4 k-steps each
             const int pb_lo = LO - pa > 0 ? LO - pa : 0, pb_hi = HI - pa < kPlanes - 1 ? HI - pa : kPlanes - 1;
             const int n_mma = (pb_hi - pb_lo + 1) * kKSteps3;
@@ -507,39 +538,45 @@ __device__ __forceinline__ void oz3_issue_pass(const Oz3Smem& sm, uint32_t tmem_
             const int n_wait = wrap ? (QMAX - (LO > 0 ? LO : 0) + 1) + 1 : ((LO - (pa + 1) >= 0) ? 2 : 1);
             auto next_wait = [&](int j) {            // j-th wait owed to the next step; the A plane comes last
                 if (!wrap) {
-                    if (LO - (pa + 1) >= 0) { if (j == 0) wait_b(cntB, LO - (pa + 1)); else wait_a(cntA + 1); }
-                    else wait_a(cntA + 1);
+                    if (LO - (pa + 1) >= 0 && j == 0) wait_b(cntB, LO - (pa + 1));
+                    else mbar_wait(&sm.fullA[san], phan);
                 } else if (more) {
-                    if (j < n_wait - 1) wait_b(cntB + QMAX + 1, QMAX - j); else wait_a(cntA + 1);
+                    if (j < n_wait - 1) wait_b(cntB + QMAX + 1, QMAX - j);
+                    else mbar_wait(&sm.fullA[san], phan);
                 }
             };
+            // the last wait is followed by kTail more MMAs of this step, so that the queue is full across the step boundary
+            constexpr int kTail = 2;
+            const int first_after = n_mma - kTail - n_wait;                  // wait j follows MMA first_after + j
 #pragma unroll
-            for (int j = 0; j < n_wait - n_mma; ++j) next_wait(j);          // more waits than MMAs: the surplus first
+            for (int j = 0; j < n_wait; ++j)
+                if (first_after + j < 0) next_wait(j);                        // more waits than MMAs: the surplus first
 #pragma unroll
             for (int w = 0; w < 4; ++w) {                                    // the window holds at most four B planes
                 const int pb = pb_lo + w;
                 if (pb > pb_hi) continue;
-                const uint32_t cb = cntB + (uint32_t)(QMAX - pb);
-                const uint32_t b_lo = b_lo0 + (cb % kNB3) * (uint32_t)(kSlotBytes3 >> 4);
+                const uint32_t b_lo = b_lo0 + ((cntB + (uint32_t)(QMAX - pb)) & (kNB3 - 1)) * kSlotLo;
 #pragma unroll
                 for (int ks = 0; ks < kKSteps3; ++ks) {
                     const int m = w * kKSteps3 + ks;
-                    if (PROBE != 2 && leader)
-                        mma_i8_n128(tmem_base + (uint32_t)((pa + pb - LO) * kTileN3), kDescHi | (a_lo + ks * (kChunk >> 4)), kDescHi | (b_lo + ks * (kChunk >> 4)),
-                                    (kc > 0 || pa > 0 || ks > 0) ? 1u : 0u);
+                    if (PROBE != 2)
+                        mma_i8_n128_if(leader, tmem_base + (uint32_t)((pa + pb - LO) * kTileN3), kDescHi | (a_lo + ks * (kChunk >> 4)),
+                                       kDescHi | (b_lo + ks * (kChunk >> 4)), (kc > 0 || pa > 0 || ks > 0) ? 1u : 0u);
                     if (m == n_mma - 1) {
                         // the step is issued: retire its A slot and the B plane that leaves the window
-                        if (leader) tc_commit(&sm.emptyA[sa_slot]);
+                        tc_commit_if(leader, &sm.emptyA[sa]);
 #pragma unroll
                         for (int q = QMAX; q >= 0; --q) {
                             const int last = HI - q < kPlanes - 1 ? HI - q : kPlanes - 1;
-                            if (last == pa && leader) tc_commit(&sm.emptyB[(cntB + (uint32_t)(QMAX - q)) % kNB3]);
+                            if (last == pa) tc_commit_if(leader, &sm.emptyB[(cntB + (uint32_t)(QMAX - q)) & (kNB3 - 1)]);
                         }
                     }
-                    const int jw = m - (n_mma - n_wait);
+                    const int jw = m - first_after;
                     if (jw >= 0 && jw < n_wait) next_wait(jw);
                 }
             }
+            sa = san;
+            pha = phan;
             ++cntA;
         }
         cntB += QMAX + 1;
@@ -551,23 +588,41 @@ __device__ __forceinline__ double i32_to_f64(int32_t v) {
     return __hiloint2double(0x43300000, (int)((uint32_t)v ^ 0x80000000u)) - 4503601774854144.0;
 }
 
-// epilogue of one pass: this warp's 32 rows x 64 columns
-template <int LO, int HI>
-__device__ __forceinline__ void oz3_epilogue_pass(uint32_t tmem_base, int quad, int half, double* crow, double w_hi) {
+// C -= tile without reading C in the SM: the negated update goes to shared memory and from there to global memory as a
+// bulk FP64 reduction (TMA, executed in L2), one 2-D box of 32 rows x 8 columns per warp and step.  The first epilogue
+// read-modify-wrote C with LDG/STG: 20 000 cycles per pass and tile (row-strided 16-byte accesses at HBM latency) in
+// which the tensor core has nothing to do, because the next pass needs the same tensor memory.  One 64-byte 1-D bulk
+// reduction per lane was no better (2048 small operations per pass: the TMA unit's issue rate); the boxed form is 64
+// operations per pass (profiles/r02_ozaki_bounds.md).
+__device__ __forceinline__ void tensor_reduce_add_2d(const CUtensorMap* map, int c0, int c1, const void* ssrc) {
+    asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2}], [%3];\n" ::"l"(reinterpret_cast<uint64_t>(map)), "r"(c0),
+                 "r"(c1), "r"(smem_u32(ssrc))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_group_read0() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_group0() { asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory"); }
+
+constexpr int kStageCols3 = 8;                                   // columns per box (64 bytes per row)
+constexpr int kStageWarpBytes3 = 32 * kStageCols3 * 8;           // one box: 32 rows x 64 B
+constexpr int kStageBytes3 = 8 * kStageWarpBytes3;               // eight epilogue warps
+
+// epilogue of one pass: this warp's 32 rows x 64 columns.  `stage` = this warp's box, (row0, col0) = its first row and
+// the tile's first column in the 2-D view of C.
+template <int LO, int HI, int PROBE = 0>
+__device__ __forceinline__ void oz3_epilogue_pass(uint32_t tmem_base, int quad, int half, int lane, const CUtensorMap* mapC, int row0, int col0, double w_hi,
+                                                  double* stage) {
     constexpr int NACC = HI - LO + 1;
 #pragma unroll 1
     for (int c0 = 64 * half; c0 < 64 * half + 64; c0 += 16) {
         int32_t v[NACC][16];
 #pragma unroll
         for (int a = 0; a < NACC; ++a) tmem_ld16(tmem_base + ((uint32_t)(32 * quad) << 16) + (uint32_t)(a * kTileN3 + c0), v[a]);
-        double2 c[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) c[j] = *reinterpret_cast<const double2*>(crow + c0 + 2 * j);
         tmem_ld_wait();
         double acc[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) acc[j] = 0.0;
-        double w = w_hi;
+        double w = -w_hi;                                               // the NEGATED update is added to C
 #pragma unroll
         for (int a = NACC - 1; a >= 0; --a) {                          // smallest weight first
 #pragma unroll
@@ -575,31 +630,38 @@ __device__ __forceinline__ void oz3_epilogue_pass(uint32_t tmem_base, int quad, 
             w *= (double)(1 << kDigitBits);
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            c[j].x -= acc[2 * j];
-            c[j].y -= acc[2 * j + 1];
-            *reinterpret_cast<double2*>(crow + c0 + 2 * j) = c[j];
+        for (int h = 0; h < 16 / kStageCols3; ++h) {
+            if (lane == 0) bulk_wait_group_read0();                     // the previous reduction has read the box
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < kStageCols3; j += 2)
+                *reinterpret_cast<double2*>(stage + lane * kStageCols3 + j) = make_double2(acc[h * kStageCols3 + j], acc[h * kStageCols3 + j + 1]);
+            fence_proxy_async_shared();
+            __syncwarp();
+            if (lane == 0) {
+                if (PROBE != 4) tensor_reduce_add_2d(mapC, col0 + c0 + h * kStageCols3, row0, stage);
+                bulk_commit_group();
+            }
         }
     }
 }
 
-// how many k-chunks before the end of a pass its C tile is prefetched into L2 (about 8 us of MMAs: long enough for HBM,
-// short enough that the operand stream does not evict it again)
-__host__ __device__ constexpr int oz3_prefetch_lead(int pass) { return pass == 0 ? 6 : 3; }
-
-// mapA / mapB: boxes of {128 bytes of k, 128 rows, 1 plane}, 128-byte swizzle.  p.kc0 / p.kchunks count 32-byte chunks and
+// mapA / mapB: boxes of {128 bytes of k, 128 rows, 1 plane}, 128-byte swizzle; mapC: FP64, the 2-D view of the output
+// array (see OzTile), boxes of {8 columns, 32 rows}, no swizzle.  p.kc0 / p.kchunks count 32-byte chunks and
 // must be multiples of 4; p.tiles_n counts 128-column tiles.  PROBE (measurement only, 0 in the product): 1 = the producers
 // skip their TMA loads (the MMAs run on whatever the slots hold), 2 = the issuer skips its MMAs (loads only), 3 = time
 // stamps of one tile of CTA 0 in g_oz3_probe.
 template <int PROBE = 0>
 __global__ void __launch_bounds__(kThreads3, 1)
-ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
+ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
+                       const __grid_constant__ CUtensorMap mapC) {
     extern __shared__ char smem_raw[];
     char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     Oz3Smem sm;
     sm.slotA = base;
     sm.slotB = base + kNA3 * kSlotBytes3;
-    sm.fullA = reinterpret_cast<uint64_t*>(base + (kNA3 + kNB3) * kSlotBytes3);
+    char* staging = base + (kNA3 + kNB3) * kSlotBytes3;
+    sm.fullA = reinterpret_cast<uint64_t*>(staging + kStageBytes3);
     sm.emptyA = sm.fullA + kNA3;
     sm.fullB = sm.emptyA + kNA3;
     sm.emptyB = sm.fullB + kNB3;
@@ -625,7 +687,7 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
 
     if (warp == 0 || warp == 10) {
         // ===== producers (whole warps, side effects by one elected lane): warp 0 streams the A planes 0 .. HI of every
-        // (pass, chunk) and prefetches the C tile into L2 shortly before the pass ends, warp 10 the B planes HI .. 0 =====
+        // (pass, chunk), warp 10 the B planes HI .. 0 =====
         const bool leader = elect_one();
         const bool isA = warp == 0;
         const CUtensorMap* map = isA ? &mapA : &mapB;
@@ -642,12 +704,7 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
             const int row = isA ? p.row0a + tm * kTileM : p.row0b + tn * kTileN3;
             for (int pass = 0; pass < 2; ++pass) {
                 const int qmax = oz3_hi(pass);
-                const int pf = nchunks > oz3_prefetch_lead(pass) ? nchunks - oz3_prefetch_lead(pass) : 0;
                 for (int kc = 0; kc < nchunks; ++kc) {
-                    if (isA && kc == pf && PROBE != 1) {
-#pragma unroll
-                        for (int r = 0; r < kTileM; r += 32) l2_prefetch_bulk(ot.c + (size_t)(r + lane) * ot.ld, kTileN3 * (uint32_t)sizeof(double));
-                    }
                     for (int i = 0; i <= qmax; ++i) {
                         const uint32_t slot = cnt % nslots;
                         mbar_wait(&empty[slot], ((cnt / nslots) & 1u) ^ 1u);
@@ -666,24 +723,24 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
         }
     } else if (warp == 1) {
         // ===== MMA issuer (whole warp; the MMAs and commits by one elected lane) =====
-        const bool leader = elect_one();
+        const uint32_t leader = elect_one() ? 1u : 0u;
         uint32_t cntA = 0, cntB = 0, tphase = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             if (!oz_tile<kTileN3>(p, tile / p.tiles_n, tile % p.tiles_n).wanted) continue;
-            const bool stamp = PROBE == 3 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && leader;
+            const bool stamp = PROBE >= 1 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && leader != 0u;
             mbar_wait(sm.tmem_empty, tphase ^ 1u);                 // the epilogue has drained the previous level sums
             tc_fence_after();
             if (stamp) g_oz3_probe[0] = clock64();
             oz3_issue_pass<oz3_lo(0), oz3_hi(0), PROBE>(sm, tmem_base, nchunks, cntA, cntB, leader);
             if (stamp) g_oz3_probe[1] = clock64();
-            if (leader) tc_commit(sm.tmem_full);
+            tc_commit_if(leader, sm.tmem_full);
             tphase ^= 1u;
             mbar_wait(sm.tmem_empty, tphase ^ 1u);
             tc_fence_after();
             if (stamp) g_oz3_probe[2] = clock64();
             oz3_issue_pass<oz3_lo(1), oz3_hi(1), PROBE>(sm, tmem_base, nchunks, cntA, cntB, leader);
             if (stamp) g_oz3_probe[3] = clock64();
-            if (leader) tc_commit(sm.tmem_full);
+            tc_commit_if(leader, sm.tmem_full);
             tphase ^= 1u;
         }
     } else {
@@ -691,21 +748,24 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
         const int quad = warp & 3, half = (warp - 2) >> 2;
         uint32_t tphase = 0;
         const double s2 = p.scale ? (*p.scale) : 1.0;
+        double* stage = reinterpret_cast<double*>(staging + (warp - 2) * kStageWarpBytes3);
+        if (lane == 0) tma_prefetch_desc(&mapC);
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const OzTile ot = oz_tile<kTileN3>(p, tile / p.tiles_n, tile % p.tiles_n);
             if (!ot.wanted) continue;
-            double* crow = ot.c + (size_t)(32 * quad + lane) * ot.ld;
 #pragma unroll
             for (int pass = 0; pass < 2; ++pass) {
                 mbar_wait(sm.tmem_full, tphase);
                 tc_fence_after();
-                const bool stamp = PROBE == 3 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && warp == 2 && lane == 0;
+                bulk_wait_group0();                                    // this lane's earlier reductions (pass 0 of this tile) are complete
+                const bool stamp = PROBE >= 1 && blockIdx.x == 0 && tile == (int)(blockIdx.x + gridDim.x) && warp == 2 && lane == 0;
                 if (stamp) g_oz3_probe[4 + 2 * pass] = clock64();
                 // weight of the last level of the pass: w_last is that of level S - 1, a level up weighs 2^bits more
                 if (pass == 0)
-                    oz3_epilogue_pass<oz3_lo(0), oz3_hi(0)>(tmem_base, quad, half, crow, p.w_last * s2 * (double)(1ull << (kDigitBits * (kPlanes - 1 - oz3_hi(0)))));
+                    oz3_epilogue_pass<oz3_lo(0), oz3_hi(0), PROBE>(tmem_base, quad, half, lane, &mapC, ot.row0 + 32 * quad, ot.col0,
+                                                                  p.w_last * s2 * (double)(1ull << (kDigitBits * (kPlanes - 1 - oz3_hi(0)))), stage);
                 else
-                    oz3_epilogue_pass<oz3_lo(1), oz3_hi(1)>(tmem_base, quad, half, crow, p.w_last * s2);
+                    oz3_epilogue_pass<oz3_lo(1), oz3_hi(1), PROBE>(tmem_base, quad, half, lane, &mapC, ot.row0 + 32 * quad, ot.col0, p.w_last * s2, stage);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(sm.tmem_empty);
@@ -713,6 +773,7 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
                 tphase ^= 1u;
             }
         }
+        bulk_wait_group0();                                            // every reduction into C has completed before the kernel ends
     }
     tc_fence_before();
     __syncthreads();

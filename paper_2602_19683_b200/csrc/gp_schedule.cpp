@@ -333,7 +333,7 @@ void build_cholesky_schedule(int M, int nbt, int workers, std::vector<SchedItem>
 
 // The FP64 part of step J of the factorisation alone (gp_cholesky_tiled_mixed): the POTRF tile task of the diagonal
 // tile (J, J) and the TRSM tile tasks of the tiles below it, for blocks that already carry J versions.
-void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk) {
+void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk, SchedStats* stats) {
     std::vector<SchedItem> prog;
     std::vector<int32_t> task;
     int32_t tid = 0;
@@ -345,11 +345,23 @@ void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedI
         for (int kk = jj + 1; kk < nbt; ++kk)
             for (int ii = kk; ii < nbt; ++ii) { emit(mk(S_UPD_L, qt + ii, qt + kk, qt + jj, qt + jj + 1)); ++tid; }
     }
+    // The TRSM tile tasks below the diagonal tile.  Inside the whole factorisation they are one chain per block row
+    // (S_ROW_L), and the trailing updates of other columns fill the gaps; here the panel is ALONE on the chip, and
+    // (M - J - 1) nbt chains of ~0.6 ms on 148 workers leave up to half of them idle in the last wave (panel 0 of
+    // n = 32768: 248 chains, 1.9 ms for 1.0 ms of work).  So a block row is emitted left-looking block by block:
+    // L(r, q) = (K(r, q) - sum_{p<q} L(r, p) L(q, p)^T) inv(L(q, q))^T as one update item and one solve item, same
+    // arithmetic and order as the chain, same version counts.
     for (int I = J + 1; I < M; ++I) {
-        for (int bi = 0; bi < nbt; ++bi) emit(mk(S_ROW_L, I * nbt + bi, qt));
+        for (int bi = 0; bi < nbt; ++bi) {
+            const int r = I * nbt + bi;
+            for (int jj = 0; jj < nbt; ++jj) {
+                if (jj > 0) emit(mk(S_UPD_L, r, qt + jj, qt, qt + jj));
+                emit(mk(S_TRSM_L, r, qt + jj));
+            }
+        }
         ++tid;
     }
-    schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, nullptr, true, J);
+    schedule(Shape(M, 0, nbt, false), prog, task, workers, blk, out, stats, true, J);
 }
 
 bool validate_panel_schedule(const std::vector<SchedItem>& items, int M, int nbt, int J) {

@@ -40,7 +40,7 @@ void build_predict_schedule(int M, int Mm, int nbt, int workers, std::vector<Sch
 
 // Step J of the factorisation without its trailing updates (the FP64 half of gp_cholesky_tiled_mixed): POTRF tile task of
 // tile (J, J) + the TRSM tile tasks below it, for blocks that already carry J versions; and its replay check.
-void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk = 128);
+void build_panel_schedule(int M, int nbt, int J, int workers, std::vector<SchedItem>& out, int blk = 128, SchedStats* stats = nullptr);
 bool validate_panel_schedule(const std::vector<SchedItem>& items, int M, int nbt, int J);
 
 // Checks that `items` is a valid execution order (every wait of every item is satisfied by items

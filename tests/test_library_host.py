@@ -172,7 +172,8 @@ def test_panel_schedules_of_the_mixed_factorisation_replay(gp, n, tile):
     for J in sorted({0, 1, M // 2, M - 1}):
         items = gp.gp_panel_schedule_selfcheck(n, tile, J)
         nbt = tile // 128
-        want = nbt + nbt * (nbt - 1) // 2 + sum((nbt - kk) for jj in range(nbt) for kk in range(jj + 1, nbt)) + (M - J - 1) * nbt
+        # diagonal tile: POTRF + TRSM + update blocks; below it every block row is nbt solves and nbt - 1 in-tile updates
+        want = nbt + nbt * (nbt - 1) // 2 + sum((nbt - kk) for jj in range(nbt) for kk in range(jj + 1, nbt)) + (M - J - 1) * nbt * (2 * nbt - 1)
         assert items == want, (J, items, want)
     assert gp.gp_panel_schedule_selfcheck(n, tile, M) == gp.ERR["SIZE"]
     assert gp.gp_mixed_workspace_bytes(n, tile) >= gp.gp_ozaki_planes() * n * n

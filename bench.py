@@ -68,6 +68,7 @@ def _parse():
                          "with one all-gather of V^T, strong scaling (SURVEY 8(e)). The last two are unmeasured on hardware.")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--cusolver-ref", action="store_true")
+    ap.add_argument("--ozaki-probe", action="store_true", help="bounds of the emulated contraction (measurement support, one JSON line)")
     return ap.parse_args()
 
 
@@ -347,7 +348,69 @@ def measure_fp64_peak(gp, torch):
     S = gp.gp_ozaki_planes()
     out["ozaki_int8_pops"] = best * (S * (S + 1) // 2) / 1e3
     del A, Ap, C
+    out["int8_mma_peak_pops"] = measure_int8_peak(gp, torch, 128)["pops"]
     return out
+
+
+def measure_int8_peak(gp, torch, n_cols):
+    """Bare tcgen05.mma kind::i8 issue loop (128 x n_cols x 32) on every SM: burst rate in int8 POPS (best of 5 launches of
+    ~1 ms) and CTA 0's cycles per MMA."""
+    cyc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    iters = 2000
+    ops = gp.gp_int8_mma_peak_launch(n_cols, iters, cyc)
+    torch.cuda.synchronize()
+    best = 0.0
+    for _ in range(5):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); gp.gp_int8_mma_peak_launch(n_cols, iters, cyc); b.record(); torch.cuda.synchronize()
+        best = max(best, ops / (a.elapsed_time(b) * 1e-3) / 1e15)
+    return {"pops": best, "cycles_per_mma": float(cyc.item()) / (16.0 * iters)}
+
+
+def run_ozaki_probe(args):
+    """Where the emulated contraction's time goes (profiles/r02_ozaki_bounds.md): the tensor core's int8 rate by a bare issue
+    loop for three MMA widths, and the 128 x 128 two-pass kernel with its parts switched off, on random and on constant
+    operands (the board's power limit makes the rate depend on how many bits toggle)."""
+    import torch
+    from paper_2602_19683_b200 import binding as gp
+    gp.load()
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    out = {"what": "bench.py --ozaki-probe", "mma_issue_loop": {}, "kernel": []}
+    for n_cols in (64, 128, 256):
+        out["mma_issue_loop"][f"128x{n_cols}x32"] = measure_int8_peak(gp, torch, n_cols)
+    S = gp.gp_ozaki_planes()
+    pairs = S * (S + 1) // 2
+    m = 8192
+    for kind in ("random", "constant"):
+        for k in (1024, 4096, 16384):
+            A = (torch.rand(m, k, dtype=torch.float64, device="cuda") - 0.5) * 1.8 if kind == "random" else torch.full((m, k), 0.3, dtype=torch.float64, device="cuda")
+            Ap = gp.gp_ozaki_slice(A, 2.0)
+            del A
+            C = torch.zeros(m, m, dtype=torch.float64, device="cuda")
+            row = {"operands": kind, "m": m, "n": m, "k": k}
+            for probe, name in ((0, "full"), (1, "no_tma_loads"), (2, "loads_only"), (4, "no_reductions_into_c")):
+                gp.gp_ozaki_probe_launch(probe, Ap, Ap, C); torch.cuda.synchronize()
+                best = 1e30
+                for _ in range(3):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(); gp.gp_ozaki_probe_launch(probe, Ap, Ap, C); b.record(); torch.cuda.synchronize()
+                    best = min(best, a.elapsed_time(b))
+                row[name] = {"ms": best, "tflops_fp64_equivalent": 2.0 * m * m * k / (best * 1e-3) / 1e12, "int8_pops": 2.0 * m * m * k * pairs / (best * 1e-3) / 1e15}
+                if probe in (1, 4) or (probe == 0 and False):
+                    pass
+                if probe != 0:
+                    t = gp.gp_ozaki_probe_stamps()
+                    mm0, mm1 = (k // 128) * 4 * sum(1 for p in range(S) for q in range(S) if p + q <= S // 2 - 1), 0
+                    mm1 = (k // 128) * 4 * pairs - mm0
+                    row[name]["stamps_cycles"] = {"pass0_issue": t[1] - t[0], "pass1_issue": t[3] - t[2], "pass0_epilogue": t[5] - t[4], "pass1_epilogue": t[7] - t[6],
+                                                  "pass0_cycles_per_mma": (t[1] - t[0]) / mm0, "pass1_cycles_per_mma": (t[3] - t[2]) / mm1}
+            out["kernel"].append(row)
+            del Ap, C
+    out["clocks"] = sampler.stop()
+    print(json.dumps(out), flush=True)
+    return 0
 
 
 LAUNCHES_PER_STEP = {"assemble": 1, "cholesky": 1, "solve": 3, "mean": 1, "full_cov": 5}   # kernels of libgp_b200.so
@@ -613,6 +676,11 @@ def run_b200(args):
                          "contraction_alone_tflops": peaks["contraction_k1024_tflops"],
                          "emulated_contraction_tflops_fp64_equivalent": peaks["ozaki_int8_contraction_fp64_equivalent_tflops"],
                          "emulated_contraction_int8_pops": peaks["ozaki_int8_pops"],
+                         "int8_mma_peak_pops": peaks["int8_mma_peak_pops"],
+                         "emulated_contraction_frac_of_int8_peak": peaks["ozaki_int8_pops"] / peaks["int8_mma_peak_pops"],
+                         "int8_peak_source": "gp_int8_mma_peak_launch: bare tcgen05.mma kind::i8 128x128x32 issue loop on every SM, burst, live "
+                                             "(MEASURED_PEAKS.json has no int8 figure; its bf16 burst x the nominal ratio 2 is given beside it)",
+                         "int8_peak_from_bf16_pops": (2.0 * mp["bf16_tflops"] / 1e3) if mp.get("bf16_tflops") else None,
                          "full_cov_exec_tflops": (n * n * m + n * m * m) / (phase["full_cov"] * 1e-3) / 1e12,
                          "hbm_gbs_measured": mp.get("hbm_gbs"),
                          "assemble_gbs": (n // tile) * (n // tile + 1) / 2 * tile * tile * 8 / (phase["assemble"] * 1e-3) / 1e9,
@@ -700,6 +768,8 @@ def main():
         return run_sweep(args)
     if args.cusolver_ref:
         return run_cusolver_ref(args)
+    if args.ozaki_probe:
+        return run_ozaki_probe(args)
     if args.mode != "replicas":
         return run_distributed(args)
     return run_b200(args)

@@ -229,6 +229,21 @@ int gp_ozaki_slice(const double* dX, int64_t rows, int64_t k, int64_t ld, double
 int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double scaleA,
                       double scaleB, double* dC, int64_t ldc, void* stream);
 
+/* Measurement support for the emulated contraction (bench.py --ozaki-probe; profiles/r02_ozaki_bounds.md).
+ *   gp_int8_mma_peak_launch: one thread per SM issues 16 * iters tcgen05.mma kind::i8 of 128 x n_cols x 32 (n_cols = 64,
+ *        128 or 256) on whatever shared memory holds; d_cycles (device, 1 entry, may be NULL) receives the clock64 ticks of
+ *        CTA 0's loop, *ops (host, may be NULL) the int8 operations of the launch (2 per multiply-add).  The caller times
+ *        the launch with events: the rate at n_cols = 128 is the int8 tensor peak bench.py holds the contraction against.
+ *   gp_ozaki_probe_launch: the 128 x 128 two-pass kernel on dense C [ma x nb] (ma, nb, k multiples of 128, k <= 16384,
+ *        scales 1) with one of its parts switched off: probe 0 = nothing (the product kernel), 1 = no TMA loads (the MMAs
+ *        run on whatever the slots hold: C is garbage), 2 = no MMAs (loads only), 4 = no reductions into C.
+ *   gp_ozaki_probe_stamps: after a launch with probe > 0 (and a synchronise), 8 clock64 stamps of the second tile of CTA 0:
+ *        pass 0 issue start / end, pass 1 issue start / end, epilogue of pass 0 start / end, epilogue of pass 1 start / end. */
+int gp_int8_mma_peak_launch(int n_cols, int iters, long long* d_cycles, double* ops, void* stream);
+int gp_ozaki_probe_launch(int probe, const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double* dC,
+                          int64_t ldc, void* stream);
+int gp_ozaki_probe_stamps(long long* h_stamps8);
+
 /* SURVEY.md 8(f) row 3, end to end: the tiled Cholesky of gp_cholesky_tiled with its trailing updates (SYRK / GEMM tile
  * tasks: > 95 % of the flops) EMULATED on the int8 tensor cores and everything on the critical path
  * (POTRF and TRSM tile tasks) in FP64 as before.  Opt-in: gp_cholesky_tiled itself is unchanged.

@@ -25,7 +25,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
-           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
+           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_int8_mma_peak_launch", "gp_ozaki_probe_launch", "gp_ozaki_probe_stamps", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
            "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n",
@@ -102,6 +102,9 @@ def load() -> ctypes.CDLL:
     lib.gp_mixed_panel.argtypes = [vp, i64, ci, ci, ci, vp, vp, sz, vp]
     lib.gp_mixed_slice_column.argtypes = [vp, i64, ci, ci, vp, sz, vp]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
+    lib.gp_int8_mma_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
+    lib.gp_ozaki_probe_launch.argtypes = [ci, vp, i64, vp, i64, i64, vp, i64, vp]
+    lib.gp_ozaki_probe_stamps.argtypes = [ctypes.POINTER(ctypes.c_longlong)]
     lib.gp_set_ozaki_tile_n.argtypes = [ci]
     lib.gp_mixed_predict_workspace_bytes.argtypes = [i64, i64, ci, psz]
     lib.gp_predict_full_cov_mixed.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
@@ -366,6 +369,26 @@ def gp_predict_full_cov_mixed(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor
     m = Xs.shape[0]
     _check(load().gp_predict_full_cov_mixed(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(Sigma),
                                             _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_full_cov_mixed")
+
+
+def gp_int8_mma_peak_launch(n_cols: int, iters: int, cycles: torch.Tensor) -> float:
+    """Enqueue the bare tcgen05.mma kind::i8 issue loop (128 x n_cols x 32) on every SM; returns its int8 operation count."""
+    ops = ctypes.c_double(0.0)
+    _check(load().gp_int8_mma_peak_launch(int(n_cols), int(iters), _ptr(cycles, torch.int64), ctypes.byref(ops), _stream()), "gp_int8_mma_peak_launch")
+    return float(ops.value)
+
+
+def gp_ozaki_probe_launch(probe: int, Aplanes: torch.Tensor, Bplanes: torch.Tensor, C: torch.Tensor) -> None:
+    _, ma, k = Aplanes.shape
+    _, nb, _ = Bplanes.shape
+    _check(load().gp_ozaki_probe_launch(int(probe), _ptr(Aplanes, torch.int8), ma, _ptr(Bplanes, torch.int8), nb, k, _ptr(C), nb, _stream()),
+           "gp_ozaki_probe_launch")
+
+
+def gp_ozaki_probe_stamps():
+    buf = (ctypes.c_longlong * 8)()
+    _check(load().gp_ozaki_probe_stamps(buf), "gp_ozaki_probe_stamps")
+    return list(buf)
 
 
 def gp_ozaki_planes() -> int:

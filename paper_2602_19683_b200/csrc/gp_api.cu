@@ -866,6 +866,19 @@ int make_plane_map(CUtensorMap* map, const int8_t* planes, uint64_t rows, uint64
 }  // namespace
 
 namespace {
+// the 2-D view [rows][ld] of an FP64 output array, boxes of {8 columns, 32 rows}: the wide kernel's bulk reductions into C
+int make_c_map(CUtensorMap* map, double* C, uint64_t ld, uint64_t rows) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return GP_ERR_CUDA;
+    const cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)(ld * sizeof(double))};
+    const cuuint32_t box[2] = {(cuuint32_t)oz::kStageCols3, 32};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, C, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? GP_OK : GP_ERR_CUDA;
+}
+
 std::atomic<int> g_ozaki_tile_n{0};       // 0 = auto (128 when the shape allows), 64, 128: gp_set_ozaki_tile_n (measurement support)
 
 // launches the emulated contraction described by q (kc0 / kchunks in 32-byte chunks) with the tile shape that fits:
@@ -882,18 +895,7 @@ int launch_ozaki(oz::OzParams q, const int8_t* planesA, uint64_t rowsA, const in
     if (wide) {
         if ((rc = make_plane_map(&mapA, planesA, rowsA, kdim, oz::kTileM, 1, oz::kChunk3)) != GP_OK) return rc;
         if ((rc = make_plane_map(&mapB, planesB, rowsB, kdim, oz::kTileN3, 1, oz::kChunk3)) != GP_OK) return rc;
-        {
-            EncodeTiledFn enc = encode_tiled();
-            if (!enc) return GP_ERR_CUDA;
-            const uint64_t ld = (q.tiled == 1 || q.tiled == 2) ? (uint64_t)q.t : (uint64_t)q.ldc;
-            const cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)c_rows};
-            const cuuint64_t strides[1] = {(cuuint64_t)(ld * sizeof(double))};
-            const cuuint32_t box[2] = {(cuuint32_t)oz::kStageCols3, 32};
-            const cuuint32_t estr[2] = {1, 1};
-            if (enc(&mapC, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, q.C, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-                return GP_ERR_CUDA;
-        }
+        if ((rc = make_c_map(&mapC, q.C, (q.tiled == 1 || q.tiled == 2) ? (uint64_t)q.t : (uint64_t)q.ldc, c_rows)) != GP_OK) return rc;
         rc = configure_once(1024u, [] {
             return cudaFuncSetAttribute(oz::ozaki_contract_kernel3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz3) == cudaSuccess;
         });
@@ -926,6 +928,69 @@ extern "C" int gp_set_ozaki_tile_n(int n) {
     if (n != 0 && n != 64 && n != 128) return GP_ERR_SIZE;
     g_ozaki_tile_n.store(n, std::memory_order_relaxed);
     return GP_OK;
+}
+
+// ---- measurement support for the emulated contraction (bench.py --ozaki-probe; profiles/r02_ozaki_bounds.md) ----
+extern "C" int gp_int8_mma_peak_launch(int n_cols, int iters, long long* d_cycles, double* ops, void* stream) {
+    if (iters <= 0 || (n_cols != 64 && n_cols != 128 && n_cols != 256)) return GP_ERR_SIZE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int grid = sm_count();
+    cudaError_t e;
+    if (n_cols == 64) {
+        e = cudaFuncSetAttribute(oz::int8_mma_peak_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemInt8Peak);
+        if (e == cudaSuccess) oz::int8_mma_peak_kernel<64><<<grid, 128, oz::kSmemInt8Peak, st>>>(iters, d_cycles);
+    } else if (n_cols == 128) {
+        e = cudaFuncSetAttribute(oz::int8_mma_peak_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemInt8Peak);
+        if (e == cudaSuccess) oz::int8_mma_peak_kernel<128><<<grid, 128, oz::kSmemInt8Peak, st>>>(iters, d_cycles);
+    } else {
+        e = cudaFuncSetAttribute(oz::int8_mma_peak_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemInt8Peak);
+        if (e == cudaSuccess) oz::int8_mma_peak_kernel<256><<<grid, 128, oz::kSmemInt8Peak, st>>>(iters, d_cycles);
+    }
+    if (e != cudaSuccess) return GP_ERR_CUDA;
+    if (ops) *ops = 2.0 * oz::kTileM * (double)n_cols * oz::kChunk * 16.0 * (double)iters * (double)grid;
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_ozaki_probe_launch(int probe, const int8_t* dAplanes, int64_t ma, const int8_t* dBplanes, int64_t nb, int64_t k, double* dC,
+                                     int64_t ldc, void* stream) {
+    if (!dAplanes || !dBplanes || !dC) return GP_ERR_NULL;
+    if (probe != 0 && probe != 1 && probe != 2 && probe != 4) return GP_ERR_MODE;
+    if (ma <= 0 || nb <= 0 || k <= 0 || ma % oz::kTileM != 0 || nb % oz::kTileN3 != 0 || k % oz::kChunk3 != 0 || k > oz::kMaxK || ldc < nb || ldc % 2 != 0)
+        return GP_ERR_SIZE;
+    oz::OzParams q;
+    memset(&q, 0, sizeof(q));
+    q.C = dC;
+    q.ldc = ldc;
+    q.tiles_m = (int)(ma / oz::kTileM);
+    q.tiles_n = (int)(nb / oz::kTileN3);
+    q.kchunks = (int)(k / oz::kChunk);
+    q.w_last = std::ldexp(1.0, -oz::kDigitBits * (oz::kPlanes + 1));
+    CUtensorMap mapA, mapB, mapC;
+    int rc;
+    if ((rc = make_plane_map(&mapA, dAplanes, (uint64_t)ma, (uint64_t)k, oz::kTileM, 1, oz::kChunk3)) != GP_OK) return rc;
+    if ((rc = make_plane_map(&mapB, dBplanes, (uint64_t)nb, (uint64_t)k, oz::kTileN3, 1, oz::kChunk3)) != GP_OK) return rc;
+    if ((rc = make_c_map(&mapC, dC, (uint64_t)ldc, (uint64_t)ma)) != GP_OK) return rc;
+    const int grid = (int)std::min<int64_t>((int64_t)q.tiles_m * q.tiles_n, sm_count());
+    cudaStream_t st = (cudaStream_t)stream;
+#define GPB_PROBE_CASE(P)                                                                                                              \
+    case P:                                                                                                                            \
+        if (cudaFuncSetAttribute(oz::ozaki_contract_kernel3<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, oz::kSmemOz3) != cudaSuccess) \
+            return GP_ERR_CUDA;                                                                                                        \
+        oz::ozaki_contract_kernel3<P><<<grid, oz::kThreads3, oz::kSmemOz3, st>>>(q, mapA, mapB, mapC);                                 \
+        break;
+    switch (probe) {
+        GPB_PROBE_CASE(0)
+        GPB_PROBE_CASE(1)
+        GPB_PROBE_CASE(2)
+        GPB_PROBE_CASE(4)
+    }
+#undef GPB_PROBE_CASE
+    return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+extern "C" int gp_ozaki_probe_stamps(long long* h_stamps8) {
+    if (!h_stamps8) return GP_ERR_NULL;
+    return cudaMemcpyFromSymbol(h_stamps8, oz::g_oz3_probe, 8 * sizeof(long long)) == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
 extern "C" int gp_ozaki_planes(void) { return oz::kPlanes; }

@@ -475,7 +475,7 @@ __device__ __forceinline__ void mma_i8_n128(uint32_t tmem_d, uint64_t desc_a, ui
     mma_i8(tmem_d, desc_a, desc_b, kIdescI8N128, accumulate);
 }
 
-__device__ long long g_oz3_probe[16];      // PROBE == 3 only: time stamps of CTA 0's first tile
+__device__ long long g_oz3_probe[8];       // PROBE > 0 only: clock64 stamps of the second tile of CTA 0
 
 struct Oz3Smem {
     char* slotA;
@@ -529,7 +529,7 @@ __device__ __forceinline__ void oz3_issue_pass(const Oz3Smem& sm, uint32_t tmem_
         for (int pa = 0; pa <= QMAX; ++pa) {
             const uint32_t san = sa + 1 == kNA3 ? 0u : sa + 1, phan = sa + 1 == kNA3 ? pha ^ 1u : pha;
             const uint32_t a_lo = a_lo0 + sa * kSlotLo;
-            if (PROBE != 6) tc_fence_after();
+            tc_fence_after();
             // this step's MMAs: pb in [max(0, LO - pa), min(S - 1, HI - pa)], 4 k-steps each
             const int pb_lo = LO - pa > 0 ? LO - pa : 0, pb_hi = HI - pa < kPlanes - 1 ? HI - pa : kPlanes - 1;
             const int n_mma = (pb_hi - pb_lo + 1) * kKSteps3;
@@ -649,8 +649,9 @@ __device__ __forceinline__ void oz3_epilogue_pass(uint32_t tmem_base, int quad, 
 // mapA / mapB: boxes of {128 bytes of k, 128 rows, 1 plane}, 128-byte swizzle; mapC: FP64, the 2-D view of the output
 // array (see OzTile), boxes of {8 columns, 32 rows}, no swizzle.  p.kc0 / p.kchunks count 32-byte chunks and
 // must be multiples of 4; p.tiles_n counts 128-column tiles.  PROBE (measurement only, 0 in the product): 1 = the producers
-// skip their TMA loads (the MMAs run on whatever the slots hold), 2 = the issuer skips its MMAs (loads only), 3 = time
-// stamps of one tile of CTA 0 in g_oz3_probe.
+// skip their TMA loads (the MMAs run on whatever the slots hold), 2 = the issuer skips its MMAs (loads only), 4 = the
+// epilogue skips its reductions into C; every PROBE > 0 leaves time stamps of the second tile of CTA 0 in g_oz3_probe
+// (pass 0: issue start, issue end; pass 1: issue start, issue end; then epilogue start / end of pass 0 and of pass 1).
 template <int PROBE = 0>
 __global__ void __launch_bounds__(kThreads3, 1)
 ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
@@ -779,6 +780,46 @@ ozaki_contract_kernel3(const __grid_constant__ OzParams p, const __grid_constant
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
 }
+
+// ---- the tensor core's int8 rate by a bare issue loop (measurement support) ---------------------------------------------
+// One thread per SM issues tcgen05.mma kind::i8 of 128 x N x 32 on whatever shared memory holds, 16 per iteration into
+// rotating accumulators; cycles[0] <- clock64 ticks of CTA 0's loop (issue to completion).  Measured on B200 at 1965 MHz:
+// N = 64: 48 cycles per MMA (the 6 KB of operands an MMA reads from shared memory at 128 B/clk), N = 128: 64, N = 256: 128
+// (= 8192 int8 MAC per cycle and SM, 4.56 POPS over the chip).  A pause of the issuing thread of up to ~100 cycles per
+// 16 MMAs is absorbed, 200 cycles cost 110: the instruction queue is about two MMAs deep.
+template <int N>
+__global__ void __launch_bounds__(128, 1) int8_mma_peak_kernel(int iters, long long* __restrict__ cycles) {
+    extern __shared__ char smem_raw[];
+    char* base = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    __shared__ uint64_t bar;
+    __shared__ uint32_t slot;
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
+    if (warp == 0) tmem_alloc(&slot, kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = slot;
+    constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+    constexpr int NACC = kTmemCols / N;
+    if (threadIdx.x == 0) {
+        const uint32_t sa = smem_u32(base), sb = sa + 4 * kSlotBytes3;
+        const long long t0 = clock64();
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                mma_i8(tmem + (uint32_t)((j % NACC) * N), smem_desc_sw128(sa + (j & 3) * kSlotBytes3 + (j >> 2) * kChunk),
+                       smem_desc_sw128(sb + ((j * 3) & 3) * (N * kChunk3) + (j >> 2) * kChunk), idesc, 1u);
+        }
+        tc_commit(&bar);
+        mbar_wait(&bar, 0);
+        if (blockIdx.x == 0 && cycles) cycles[0] = clock64() - t0;
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, kTmemCols);
+}
+constexpr int kSmemInt8Peak = 4 * kSlotBytes3 + 4 * 256 * kChunk3 + 2048;
 
 }  // namespace oz
 }  // namespace gpb

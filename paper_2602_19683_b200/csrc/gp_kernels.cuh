@@ -298,6 +298,9 @@ __device__ __forceinline__ int ld_acquire_i(const int* p) {
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void solve_release_flag(int* p) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;\n" ::"l"(p), "r"(1) : "memory");
+}
 __device__ __forceinline__ void cp_async16_solve(void* smem_dst, const void* gmem_src) {
     unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
@@ -359,7 +362,7 @@ __global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __r
             l[r][1] = __ldcs(row + 1);
         }
         if (lane == 0) {                     // (c) ... then the wait for x_p, per warp
-            while (ld_acquire_i(flags + pb) == 0) __nanosleep(20);
+            while (ld_acquire_i(flags + pb) == 0) { }
         }
         __syncwarp();
         const double2 x01 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx));
@@ -393,9 +396,10 @@ __global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __r
 #pragma unroll
         for (int r = 0; r < RPT; ++r) x[(size_t)i * SB + ty + TY * r] = part[r];
     }
-    __threadfence();
+    // publish: the CTA barrier orders every thread's stores of x_i before thread 0, whose release makes them visible at
+    // gpu scope before the flag moves (the two MEMBAR.SC per thread of __threadfence cost ~1 us of a ~4 us chain step)
     __syncthreads();
-    if (tid == 0) { __threadfence(); atomicExch(flags + i, 1); }
+    if (tid == 0) solve_release_flag(flags + i);
 }
 
 // Backward: x_j = invD_j^T (b_j - sum_{i>j} L(i,j)^T x_i); block columns handed out from the last.
@@ -431,7 +435,7 @@ __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __
             l[r][1] = __ldcs(row + 1);
         }
         if (lane == 0) {
-            while (ld_acquire_i(flags + ib) == 0) __nanosleep(20);
+            while (ld_acquire_i(flags + ib) == 0) { }
         }
         __syncwarp();
 #pragma unroll
@@ -475,9 +479,8 @@ __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __
         for (int k = 0; k < TY; ++k) s += s_part[k * SB + tid];
         x[(size_t)j * SB + tid] = s;
     }
-    __threadfence();
     __syncthreads();
-    if (tid == 0) { __threadfence(); atomicExch(flags + j, 1); }
+    if (tid == 0) solve_release_flag(flags + j);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -169,3 +169,42 @@ def test_mixed_prediction_matches_oracle(gp, n, m, D, tile):
     assert np.array_equal(S, S.T)
     d = np.diag(S)
     assert d.min() >= 0.0 and d.max() <= h.vertical
+
+
+# ---------------------------------------------------------------- measurement support
+def test_int8_mma_issue_loop_reports_the_tensor_core_rate(gp):
+    """gp_int8_mma_peak_launch: cycles per 128 x N x 32 MMA of CTA 0 (N = 64 is bound by the shared-memory operand read
+    at 48, N = 128 and 256 run at the pipe's 8192 MAC per cycle: 64 and 128)."""
+    cyc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for n_cols, want in ((64, 48.0), (128, 64.0), (256, 128.0)):
+        iters = 500
+        ops = gp.gp_int8_mma_peak_launch(n_cols, iters, cyc)
+        torch.cuda.synchronize()
+        assert ops == 2.0 * 128 * n_cols * 32 * 16 * iters * torch.cuda.get_device_properties(0).multi_processor_count
+        per = float(cyc.item()) / (16.0 * iters)
+        assert want * 0.98 <= per <= want * 1.15, (n_cols, per)
+    with pytest.raises(gp.GpError):
+        gp.gp_int8_mma_peak_launch(96, 10, cyc)
+
+
+def test_probe_launch_without_a_switch_is_the_product_kernel(gp):
+    """gp_ozaki_probe_launch(0) = the 128 x 128 two-pass kernel on dense C with scales 1: same bits as gp_ozaki_contract;
+    with the loads or the reductions switched off it still terminates and leaves its time stamps."""
+    rng = np.random.default_rng(11)
+    m, k = 384, 512
+    A = torch.from_numpy(rng.uniform(-0.45, 0.45, size=(m, k))).cuda()
+    planes = gp.gp_ozaki_slice(A, 1.0)
+    C0 = torch.from_numpy(rng.normal(size=(m, m))).cuda()
+    C1, C2 = C0.clone(), C0.clone()
+    gp.gp_ozaki_contract(planes, planes, 1.0, 1.0, C1)
+    gp.gp_ozaki_probe_launch(0, planes, planes, C2)
+    torch.cuda.synchronize()
+    assert torch.equal(C1, C2)
+    assert relerr(C1.cpu().numpy(), (C0 - A @ A.T).cpu().numpy()) <= 1e-14
+    for probe in (1, 2, 4):
+        gp.gp_ozaki_probe_launch(probe, planes, planes, C2)
+        torch.cuda.synchronize()
+        t = gp.gp_ozaki_probe_stamps()
+        assert len(t) == 8
+    with pytest.raises(gp.GpError):
+        gp.gp_ozaki_probe_launch(3, planes, planes, C2)

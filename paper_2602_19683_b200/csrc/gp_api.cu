@@ -229,26 +229,26 @@ int launch_exec_any(int b, const ExecParams& p, int64_t m, int workers, cudaStre
 }
 
 template <int BLK>
-int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStream_t st) {
+int launch_trtri(const double* L, int t, int nbt, int NB, double* invD, cudaStream_t st, double* fill = nullptr) {
     constexpr int smem = DiagSmem<BLK>::kBytes;
     const int rc = configure_once(BLK == 128 ? KB_TRTRI128 : (BLK == 64 ? KB_TRTRI64 : KB_TRTRI32), [] {
         return cudaFuncSetAttribute(trtri_diag_kernel<BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
     });
     if (rc != GP_OK) return rc;
-    trtri_diag_kernel<BLK><<<NB, kConsumerThreads, smem, st>>>(L, t, nbt, invD);
+    trtri_diag_kernel<BLK><<<NB, kConsumerThreads, smem, st>>>(L, t, nbt, invD, fill);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
-int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaStream_t st) {
+int launch_trtri_any(int b, const double* L, int t, int NB, double* invD, cudaStream_t st, double* fill = nullptr) {
     switch (b) {
-        case 128: return launch_trtri<128>(L, t, t / 128, NB, invD, st);
-        case 64: return launch_trtri<64>(L, t, t / 64, NB, invD, st);
-        default: return launch_trtri<32>(L, t, t / 32, NB, invD, st);
+        case 128: return launch_trtri<128>(L, t, t / 128, NB, invD, st, fill);
+        case 64: return launch_trtri<64>(L, t, t / 64, NB, invD, st, fill);
+        default: return launch_trtri<32>(L, t, t / 32, NB, invD, st, fill);
     }
 }
 
 template <int SB>
-int launch_solves(const double* dL, int tile, int NB, const double* invD, const double* dY, double* beta, double* dAlpha, int* flags,
+int launch_solves(const double* dL, int tile, int NB, const double* invD, const double* dY, double* beta, double* dAlpha,
                   unsigned int* ticket, cudaStream_t st) {
     constexpr int smem = SolveCfg<SB>::kSmemBytes;
     const int rc = configure_once(SB == 128 ? KB_SOLVE128 : (SB == 64 ? KB_SOLVE64 : KB_SOLVE32), [] {
@@ -256,8 +256,8 @@ int launch_solves(const double* dL, int tile, int NB, const double* invD, const 
                cudaFuncSetAttribute(backward_solve_kernel<SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) == cudaSuccess;
     });
     if (rc != GP_OK) return rc;
-    forward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, dY, beta, flags, ticket);
-    backward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, beta, dAlpha, flags + NB, ticket + 1);
+    forward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, dY, beta, dAlpha, ticket);
+    backward_solve_kernel<SB><<<NB, 256, smem, st>>>(dL, tile, NB, invD, beta, dAlpha, ticket + 1);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
 }
 
@@ -457,14 +457,14 @@ int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dA
     if (cudaMemsetAsync(ws, 0, w.beta, st) != cudaSuccess) return GP_ERR_CUDA;
     double* invD = (double*)(ws + w.invD);
     double* beta = dBeta ? dBeta : (double*)(ws + w.beta);
-    int* flags = (int*)(ws + w.flags);
     unsigned int* ticket = (unsigned int*)(ws + w.ticket);
-    rc = launch_trtri_any(b, dL, tile, NB, invD, st);
+    // the kernel that inverts the diagonal blocks also marks beta "not yet computed" (the forward solve marks alpha)
+    rc = launch_trtri_any(b, dL, tile, NB, invD, st, beta);
     if (rc != GP_OK) return rc;
     switch (b) {
-        case 128: rc = launch_solves<128>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
-        case 64: rc = launch_solves<64>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
-        default: rc = launch_solves<32>(dL, tile, NB, invD, dY, beta, dAlpha, flags, ticket, st); break;
+        case 128: rc = launch_solves<128>(dL, tile, NB, invD, dY, beta, dAlpha, ticket, st); break;
+        case 64: rc = launch_solves<64>(dL, tile, NB, invD, dY, beta, dAlpha, ticket, st); break;
+        default: rc = launch_solves<32>(dL, tile, NB, invD, dY, beta, dAlpha, ticket, st); break;
     }
     if (rc != GP_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;

@@ -451,11 +451,14 @@ exec_kernel(const __grid_constant__ ExecParams p, const __grid_constant__ CUtens
 
 // Batched inverse of the diagonal blocks of L (used by gp_solve and gp_predict_full_cov, which
 // receive only L): one CTA of kConsumerThreads per diagonal block.
+// `fill` (may be null): a vector of gridDim.x * BLK doubles whose block q is overwritten with the "not yet computed" pattern
+// of the solve kernels (gp_kernels.cuh: kSolvePending), so that gp_solve needs no extra launch for it.
 template <int BLK>
 __global__ void __launch_bounds__(kConsumerThreads, 1) trtri_diag_kernel(const double* __restrict__ L, int t, int nbt,
-                                                                          double* __restrict__ invD) {
+                                                                          double* __restrict__ invD, double* __restrict__ fill) {
     extern __shared__ __align__(16) double smem[];
     const int q = blockIdx.x;
+    if (fill != nullptr && threadIdx.x < BLK) fill[(size_t)q * BLK + threadIdx.x] = __longlong_as_double(kSolvePending);
     const int I = q / nbt;
     const double* G = L + ((size_t)I * (I + 1) / 2 + I) * (size_t)t * t + (size_t)(q % nbt) * BLK * t + (size_t)(q % nbt) * BLK;
     trtri_block<BLK>(smem, G, t, invD + (size_t)q * BLK * BLK);

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "gp_tma.cuh"
+
 namespace gpb {
 
 struct HyperDev {
@@ -298,9 +300,19 @@ __device__ __forceinline__ int ld_acquire_i(const int* p) {
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void solve_release_flag(int* p) {
-    asm volatile("st.release.gpu.global.s32 [%0], %1;\n" ::"l"(p), "r"(1) : "memory");
+// relaxed gpu-scope accesses to the published solution: they go to L2, where every SM sees them
+__device__ __forceinline__ double2 solve_ld2(const double* p) {
+    double2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
 }
+__device__ __forceinline__ double solve_ld1(const double* p) {
+    double v;
+    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];\n" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void solve_st1(double* p, double v) { asm volatile("st.relaxed.gpu.global.f64 [%0], %1;\n" ::"l"(p), "d"(v) : "memory"); }
+__device__ __forceinline__ bool solve_pending(double v) { return __double_as_longlong(v) == kSolvePending; }
 __device__ __forceinline__ void cp_async16_solve(void* smem_dst, const void* gmem_src) {
     unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
@@ -317,6 +329,11 @@ struct SolveCfg {
     static constexpr int TX = SB / 4;             // threads across a row (4 columns each); divides 32
     static constexpr int TY = 256 / TX;           // row groups
     static constexpr int RPT = SB / TY;           // rows per thread
+    // blocks of L in flight per CTA (register buffers of RPT x 4 doubles each).  More than one was measured for the 64- and
+    // 32-row kernels (4 in flight): c2 0.396 -> 0.381 ms, c1 0.065 -> 0.069 ms, c3 with 64-row blocks 2.31 -> 2.66 ms: the
+    // solves are not bound by the latency of a CTA's own stream (at c3 they move 4 TB/s, 62 % of the measured HBM rate,
+    // at the smaller sizes the chain of diagonal steps is the bound), so one block in flight it stays.
+    static constexpr int PD = 1;
     static constexpr int kSmemBytes = SB * SB * 8 + SB * 8 + TY * SB * 8;   // invD, rhs, cross-warp partials
 };
 
@@ -332,14 +349,15 @@ __device__ __forceinline__ double group_sum(double v) {
 template <int SB>
 __global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __restrict__ L, int t, int NB,
                                                                const double* __restrict__ invD, const double* __restrict__ y,
-                                                               double* x, int* flags, unsigned int* ticket) {
+                                                               double* x, double* next_x, unsigned int* ticket) {
     using Cfg = SolveCfg<SB>;
     constexpr int TX = Cfg::TX, TY = Cfg::TY, RPT = Cfg::RPT;
     extern __shared__ __align__(16) double sm[];
     double* s_inv = sm;                 // SB x SB, row-major
     double* s_rhs = sm + SB * SB;       // SB
     __shared__ unsigned int s_row;
-    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX, lane = tid & 31;
+    __shared__ __align__(16) double s_x[2][SB];
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
     const int sbt = t / SB;
     if (tid == 0) s_row = atomicAdd(ticket, 1u);
     __syncthreads();
@@ -352,27 +370,48 @@ __global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __r
     double acc[RPT];
 #pragma unroll
     for (int r = 0; r < RPT; ++r) acc[r] = 0.0;
-    for (int pb = 0; pb < i; ++pb) {
+    constexpr int PD = Cfg::PD;
+    double2 l[PD][RPT][2];
+    auto load_block = [&](int slot, int pb) {      // (b) the blocks of L first ...
         const double* blk = tile_block_ptr(L, t, sbt, i, pb, SB);
-        double2 l[RPT][2];
-#pragma unroll
-        for (int r = 0; r < RPT; ++r) {      // (b) the block of L first ...
-            const double2* row = reinterpret_cast<const double2*>(blk + (size_t)(ty + TY * r) * t + 4 * tx);
-            l[r][0] = __ldcs(row);
-            l[r][1] = __ldcs(row + 1);
-        }
-        if (lane == 0) {                     // (c) ... then the wait for x_p, per warp
-            while (ld_acquire_i(flags + pb) == 0) { }
-        }
-        __syncwarp();
-        const double2 x01 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx));
-        const double2 x23 = __ldcg(reinterpret_cast<const double2*>(x + (size_t)pb * SB + 4 * tx + 2));
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
-            acc[r] = fma(l[r][0].x, x01.x, acc[r]);
-            acc[r] = fma(l[r][0].y, x01.y, acc[r]);
-            acc[r] = fma(l[r][1].x, x23.x, acc[r]);
-            acc[r] = fma(l[r][1].y, x23.y, acc[r]);
+            const double2* row = reinterpret_cast<const double2*>(blk + (size_t)(ty + TY * r) * t + 4 * tx);
+            l[slot][r][0] = __ldcs(row);
+            l[slot][r][1] = __ldcs(row + 1);
+        }
+    };
+#pragma unroll
+    for (int sl = 0; sl < PD; ++sl)
+        if (sl < i) load_block(sl, sl);
+    for (int pb0 = 0; pb0 < i; pb0 += PD) {
+#pragma unroll
+        for (int sl = 0; sl < PD; ++sl) {
+            const int pb = pb0 + sl;
+            if (pb >= i) break;
+            // (c) ... then the wait for x_p.  ONE warp polls the values (its lanes cover the whole piece) and hands them to
+            // the others through shared memory: with every warp of every CTA polling, the L2 slice that holds x_p was
+            // crowded (c3: 2.8 ms instead of 2.3), and a back-off costs more than it saves (__nanosleep is coarse: 4.9 ms).
+            double* sx = s_x[pb & 1];
+            if (tid < SB / 4) {
+                double2 p01, p23;
+                do {
+                    p01 = solve_ld2(x + (size_t)pb * SB + 4 * tid);
+                    p23 = solve_ld2(x + (size_t)pb * SB + 4 * tid + 2);
+                } while (solve_pending(p01.x) || solve_pending(p01.y) || solve_pending(p23.x) || solve_pending(p23.y));
+                *reinterpret_cast<double2*>(sx + 4 * tid) = p01;
+                *reinterpret_cast<double2*>(sx + 4 * tid + 2) = p23;
+            }
+            __syncthreads();     // one barrier per block: the buffer written two blocks later is read before the next barrier
+            const double2 x01 = *reinterpret_cast<const double2*>(sx + 4 * tx), x23 = *reinterpret_cast<const double2*>(sx + 4 * tx + 2);
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                acc[r] = fma(l[sl][r][0].x, x01.x, acc[r]);
+                acc[r] = fma(l[sl][r][0].y, x01.y, acc[r]);
+                acc[r] = fma(l[sl][r][1].x, x23.x, acc[r]);
+                acc[r] = fma(l[sl][r][1].y, x23.y, acc[r]);
+            }
+            if (pb + PD < i) load_block(sl, pb + PD);
         }
     }
 #pragma unroll
@@ -394,19 +433,18 @@ __global__ void __launch_bounds__(256, 1) forward_solve_kernel(const double* __r
     for (int r = 0; r < RPT; ++r) part[r] = group_sum<TX>(part[r]);
     if (tx == 0) {
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) x[(size_t)i * SB + ty + TY * r] = part[r];
+        for (int r = 0; r < RPT; ++r) solve_st1(x + (size_t)i * SB + ty + TY * r, part[r]);   // published by value: no flag, no fence
     }
-    // publish: the CTA barrier orders every thread's stores of x_i before thread 0, whose release makes them visible at
-    // gpu scope before the flag moves (the two MEMBAR.SC per thread of __threadfence cost ~1 us of a ~4 us chain step)
-    __syncthreads();
-    if (tid == 0) solve_release_flag(flags + i);
+    // y_i has been consumed (only this CTA reads it): mark block i of the backward solve's output "not yet computed"
+    // (next_x may alias y)
+    if (next_x != nullptr && tid < SB) next_x[(size_t)i * SB + tid] = __longlong_as_double(kSolvePending);
 }
 
 // Backward: x_j = invD_j^T (b_j - sum_{i>j} L(i,j)^T x_i); block columns handed out from the last.
 template <int SB>
 __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __restrict__ L, int t, int NB,
                                                                 const double* __restrict__ invD, const double* __restrict__ b,
-                                                                double* x, int* flags, unsigned int* ticket) {
+                                                                double* x, unsigned int* ticket) {
     using Cfg = SolveCfg<SB>;
     constexpr int TX = Cfg::TX, TY = Cfg::TY, RPT = Cfg::RPT;
     extern __shared__ __align__(16) double sm[];
@@ -414,7 +452,8 @@ __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __
     double* s_rhs = sm + SB * SB;                // SB
     double* s_part = sm + SB * SB + SB;          // TY x SB partial column sums
     __shared__ unsigned int s_col;
-    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX, lane = tid & 31;
+    __shared__ __align__(16) double s_x[2][SB];
+    const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
     const int sbt = t / SB;
     if (tid == 0) s_col = atomicAdd(ticket, 1u);
     __syncthreads();
@@ -425,26 +464,45 @@ __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __
         for (int idx = tid; idx < SB * SB / 2; idx += 256) cp_async16_solve(s_inv + 2 * idx, inv + 2 * idx);
     }
     double acc[4] = {0.0, 0.0, 0.0, 0.0};        // columns 4tx..4tx+3, partial over this thread's rows
-    for (int ib = NB - 1; ib > j; --ib) {
+    constexpr int PD = Cfg::PD;
+    double2 l[PD][RPT][2];
+    auto load_block = [&](int slot, int ib) {
         const double* blk = tile_block_ptr(L, t, sbt, ib, j, SB);
-        double2 l[RPT][2];
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
             const double2* row = reinterpret_cast<const double2*>(blk + (size_t)(ty + TY * r) * t + 4 * tx);
-            l[r][0] = __ldcs(row);
-            l[r][1] = __ldcs(row + 1);
+            l[slot][r][0] = __ldcs(row);
+            l[slot][r][1] = __ldcs(row + 1);
         }
-        if (lane == 0) {
-            while (ld_acquire_i(flags + ib) == 0) { }
-        }
-        __syncwarp();
+    };
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) {
-            const double xv = __ldcg(x + (size_t)ib * SB + ty + TY * r);
-            acc[0] = fma(l[r][0].x, xv, acc[0]);
-            acc[1] = fma(l[r][0].y, xv, acc[1]);
-            acc[2] = fma(l[r][1].x, xv, acc[2]);
-            acc[3] = fma(l[r][1].y, xv, acc[3]);
+    for (int sl = 0; sl < PD; ++sl)
+        if (NB - 1 - sl > j) load_block(sl, NB - 1 - sl);
+    for (int ib0 = NB - 1; ib0 > j; ib0 -= PD) {
+#pragma unroll
+        for (int sl = 0; sl < PD; ++sl) {
+            const int ib = ib0 - sl;
+            if (ib <= j) break;
+            double* sx = s_x[ib & 1];            // x_ib: polled by value by one warp, handed over through shared memory
+            if (tid < SB / 4) {
+                double2 p01, p23;
+                do {
+                    p01 = solve_ld2(x + (size_t)ib * SB + 4 * tid);
+                    p23 = solve_ld2(x + (size_t)ib * SB + 4 * tid + 2);
+                } while (solve_pending(p01.x) || solve_pending(p01.y) || solve_pending(p23.x) || solve_pending(p23.y));
+                *reinterpret_cast<double2*>(sx + 4 * tid) = p01;
+                *reinterpret_cast<double2*>(sx + 4 * tid + 2) = p23;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const double xv = sx[ty + TY * r];
+                acc[0] = fma(l[sl][r][0].x, xv, acc[0]);
+                acc[1] = fma(l[sl][r][0].y, xv, acc[1]);
+                acc[2] = fma(l[sl][r][1].x, xv, acc[2]);
+                acc[3] = fma(l[sl][r][1].y, xv, acc[3]);
+            }
+            if (ib - PD > j) load_block(sl, ib - PD);
         }
     }
 #pragma unroll
@@ -477,10 +535,8 @@ __global__ void __launch_bounds__(256, 1) backward_solve_kernel(const double* __
         double s = 0.0;
 #pragma unroll
         for (int k = 0; k < TY; ++k) s += s_part[k * SB + tid];
-        x[(size_t)j * SB + tid] = s;
+        solve_st1(x + (size_t)j * SB + tid, s);
     }
-    __syncthreads();
-    if (tid == 0) solve_release_flag(flags + j);
 }
 
 // ---------------------------------------------------------------------------------------------

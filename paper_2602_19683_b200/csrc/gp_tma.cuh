@@ -109,6 +109,12 @@ __device__ __forceinline__ void red_release_add(int* p, int v) {
     asm volatile("red.release.gpu.global.add.s32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
 }
 
+// "Not yet computed" mark of the triangular solves (gp_kernels.cuh): the pieces of x are published by their VALUES, a
+// consumer polls the doubles it needs until none of them carries this bit pattern -- one L2 round trip where a flag plus
+// a load of x are two.  The pattern is a SIGNALLING NaN: arithmetic never produces one (NaN results are quiet, and a
+// signalling payload that enters through the inputs is quieted by the first operation), so no computed x can equal it.
+constexpr long long kSolvePending = (long long)0xFFF4DEADBEEF5EEDull;
+
 __device__ __forceinline__ int ld_acquire(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");

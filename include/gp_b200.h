@@ -97,6 +97,8 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
 /* Forward and backward substitution -- PAPER.md:72: L beta = y, then L^T alpha = beta; steps a7-a8.
  *   dL: lower-packed tiles of L.  dY [n].  dAlpha [n] <- K^-1 y.
  *   dBeta [n] <- L^-1 y; may be NULL, then dWork must hold n doubles more (see gp_workspace_bytes).
+ *   dAlpha may be the same buffer as dY (y is consumed before alpha is written); dBeta must not overlap dY or dAlpha
+ *   (it is marked "not yet computed" before y is read: the pieces of a solution are published by their values).
  *   dWork/work_bytes: scratch, at least the `solve` size from gp_workspace_bytes(). */
 int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta,
              void* dWork, size_t work_bytes, void* stream);

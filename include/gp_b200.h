@@ -275,6 +275,17 @@ int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, int k_tile0,
 int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
                    void* stream);
 int gp_mixed_slice_column(const double* dKL, int64_t n, int tile, int J, void* dWork, size_t work_bytes, void* stream);
+/* gp_mixed_panel with the panel broadcast FUSED into it ("per step the owner factors the panel and
+ * broadcasts ... fused as the epilogue of the TRSM kernel"): every block of tile column J that the step finishes (the
+ * diagonal blocks by POTRF, the blocks below by their solve) is stored not only into dKL but also at the same offset of
+ * peers[0 .. npeers-1] (host array of DEVICE addresses, npeers <= 7): the other ranks' copies of the tile array, mapped into
+ * this GPU's address space (NVLink peer memory after cudaIpcOpenMemHandle + cudaDeviceEnablePeerAccess; other buffers of
+ * the same device in the one-GPU emulation of tests/test_gpu_multi.py).  The transfer rides on the panel step block by
+ * block instead of following it as a collective; the stores are complete when the call's work on `stream` is, so the
+ * receivers need one barrier after it and no copy.  The strict upper part of the diagonal tile is not transferred
+ * (it is never read).  npeers = 0 is gp_mixed_panel. */
+int gp_mixed_panel_bcast(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                         double* const* peers, int npeers, void* stream);
 
 /* The full-covariance prediction on the same emulated contraction (opt-in; gp_predict_full_cov is unchanged): the
  * V^T solve left-looking over tile columns (column P gets V^T(:,0:P) L(P,0:P)^T in one emulated contraction, then its FP64

@@ -25,7 +25,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
-           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_int8_mma_peak_launch", "gp_ozaki_probe_launch", "gp_ozaki_probe_stamps", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
+           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_mixed_panel_bcast", "gp_int8_mma_peak_launch", "gp_ozaki_probe_launch", "gp_ozaki_probe_stamps", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
            "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n",
@@ -101,6 +101,7 @@ def load() -> ctypes.CDLL:
     lib.gp_mixed_update_column.argtypes = [vp, i64, ci, ci, ci, ci, vp, sz, vp]
     lib.gp_mixed_panel.argtypes = [vp, i64, ci, ci, ci, vp, vp, sz, vp]
     lib.gp_mixed_slice_column.argtypes = [vp, i64, ci, ci, vp, sz, vp]
+    lib.gp_mixed_panel_bcast.argtypes = [vp, i64, ci, ci, ci, vp, vp, sz, ctypes.POINTER(ctypes.c_void_p), ci, vp]
     lib.gp_ozaki_plane_bytes.argtypes = [i64, i64, psz]
     lib.gp_int8_mma_peak_launch.argtypes = [ci, ci, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.gp_ozaki_probe_launch.argtypes = [ci, vp, i64, vp, i64, i64, vp, i64, vp]
@@ -347,6 +348,14 @@ def gp_mixed_update_column(KL: torch.Tensor, n: int, tile: int, J: int, k0: int,
 def gp_mixed_panel(KL: torch.Tensor, n: int, tile: int, J: int, sched_width: int, info: torch.Tensor, work: torch.Tensor) -> None:
     _check(load().gp_mixed_panel(_ptr(KL), n, tile, J, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8), work.numel(),
                                  _stream()), "gp_mixed_panel")
+
+
+def gp_mixed_panel_bcast(KL: torch.Tensor, n: int, tile: int, J: int, sched_width: int, info: torch.Tensor, work: torch.Tensor, peers) -> None:
+    """gp_mixed_panel whose finished blocks are also stored into the other ranks' copies of the tile array: `peers` = their
+    device addresses as seen from this GPU (ints; at most 7)."""
+    arr = (ctypes.c_void_p * max(len(peers), 1))(*[ctypes.c_void_p(int(a)) for a in peers])
+    _check(load().gp_mixed_panel_bcast(_ptr(KL), n, tile, J, sched_width, _ptr(info, torch.int32), _ptr(work, torch.uint8), work.numel(),
+                                       arr, len(peers), _stream()), "gp_mixed_panel_bcast")
 
 
 def gp_mixed_slice_column(KL: torch.Tensor, n: int, tile: int, J: int, work: torch.Tensor) -> None:

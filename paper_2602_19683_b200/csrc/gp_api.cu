@@ -1145,9 +1145,13 @@ extern "C" int gp_mixed_update_column(double* dKL, int64_t n, int tile, int J, i
     return launch_ozaki(q, planes, (uint64_t)n, planes, (uint64_t)n, (uint64_t)n, tile, (uint64_t)c.M * (c.M + 1) / 2 * (uint64_t)tile, c.st);
 }
 
-extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
-                              void* stream) {
+namespace {
+int mixed_panel_impl(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes, double* const* peers,
+                     int npeers, void* stream) {
     if (!dKL || !d_info) return GP_ERR_NULL;
+    if (npeers < 0 || npeers > kMaxPeers || (npeers > 0 && !peers)) return GP_ERR_SIZE;
+    for (int k = 0; k < npeers; ++k)
+        if (!peers[k] || peers[k] == dKL) return GP_ERR_NULL;
     MixedCtx c;
     int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
     if (rc != GP_OK) return rc;
@@ -1169,12 +1173,25 @@ extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched
     p.items = cs.d_items;
     p.nitems = cs.nitems;
     p.ticket = (unsigned int*)(c.ws + c.w.ticket) + J;
+    p.npeers = npeers;
+    for (int k = 0; k < npeers; ++k) p.peerL[k] = peers[k];
     ExecMaps mp;
     if ((rc = make_exec_maps(&mp, p, 128, 0)) != GP_OK) return rc;
     // the J trailing updates of this column were applied by the emulated contraction, outside the executor's counters
     if (cudaMemsetAsync(p.ticket, 0, sizeof(unsigned int), c.st) != cudaSuccess) return GP_ERR_CUDA;
     oz::set_column_versions_kernel<<<(c.NB * c.nbt + 255) / 256, 256, 0, c.st>>>(p.verL, c.NB, c.nbt, J, kConsumerWarps);
     return launch_exec<128>(p, mp, workers_for(sched_width), c.st);
+}
+}  // namespace
+
+extern "C" int gp_mixed_panel(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                              void* stream) {
+    return mixed_panel_impl(dKL, n, tile, J, sched_width, d_info, dWork, work_bytes, nullptr, 0, stream);
+}
+
+extern "C" int gp_mixed_panel_bcast(double* dKL, int64_t n, int tile, int J, int sched_width, int* d_info, void* dWork, size_t work_bytes,
+                                    double* const* peers, int npeers, void* stream) {
+    return mixed_panel_impl(dKL, n, tile, J, sched_width, d_info, dWork, work_bytes, peers, npeers, stream);
 }
 
 extern "C" int gp_mixed_slice_column(const double* dKL, int64_t n, int tile, int J, void* dWork, size_t work_bytes, void* stream) {

@@ -59,6 +59,8 @@ struct Item {              // 16 bytes
     uint32_t q;            // q0 | (q1 << 16): contraction block range (UPD_*)
 };
 
+constexpr int kMaxPeers = 7;
+
 struct ExecParams {
     double* L;             // lower-packed tiles (n x n)
     double* Vt;            // general tiles (m x n), or nullptr
@@ -84,6 +86,13 @@ struct ExecParams {
     int L_final;           // 1: L is an input that is final everywhere (predictor), no waits on it
     int no_deps;           // 1: skip every dependency wait (contraction microbenchmark only)
     unsigned long long* stats;   // 8 per worker CTA, see gp_exec_stats in include/gp_b200.h
+    // Fused panel broadcast ("broadcast ... fused as the epilogue of the TRSM kernel"): every block of L
+    // that a job FINISHES (POTRF of a diagonal block, the solve of a block below it) is also stored at the same offset of
+    // npeers other tile arrays -- the copies of L the other ranks hold, mapped into this GPU's address space (NVLink peer
+    // memory; in the one-GPU emulation other buffers of the same device).  The transfer rides on the panel step block by
+    // block instead of following it as a separate collective.  0 peers: nothing changes.
+    double* peerL[kMaxPeers];
+    int npeers;
 };
 
 enum JobKind : int { JOB_GEMM_SUB = 0, JOB_GEMM_SET = 1, JOB_POTRF = 2, JOB_EXIT = 3 };
@@ -357,6 +366,16 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
             fence_proxy_async_global();      // L(q,q), invD(q): read by other CTAs' TMA
             fence_proxy_async_shared();      // the ring is about to be overwritten by TMA again
             cbar();
+            if (p.npeers > 0) {              // the finished diagonal block goes to the other ranks' copies of L
+                const size_t off = (size_t)(j.C - p.L);
+                for (int k = 0; k < p.npeers; ++k) {
+                    double* dst = p.peerL[k] + off;
+                    for (int idx = threadIdx.x; idx < BLK * BLK / 2; idx += kConsumerThreads) {
+                        const int r = idx / (BLK / 2), c2 = idx % (BLK / 2);
+                        __stcg(reinterpret_cast<double2*>(dst + (size_t)r * j.ldc) + c2, __ldcg(reinterpret_cast<const double2*>(j.C + (size_t)r * j.ldc) + c2));
+                    }
+                }
+            }
             if (threadIdx.x == 0) red_release_add(j.sig, kConsumerWarps);
             continue;
         }
@@ -383,6 +402,10 @@ __device__ void consumer_loop(const ExecParams& p, char* base) {
             if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
         store_tile<BLK>(j.C, j.ldc, j.kind, w, acc);
+        if (j.kind == JOB_GEMM_SET && p.npeers > 0) {       // a solved block of L is final: the other ranks' copies get it too
+            const size_t off = (size_t)(j.C - p.L);
+            for (int k = 0; k < p.npeers; ++k) store_tile<BLK>(p.peerL[k] + off, j.ldc, JOB_GEMM_SET, w, acc);
+        }
         fence_proxy_async_global();          // this warp's part of C: read by TMA later
         __syncwarp();
         if (lane == 0) red_release_add(j.sig, j.arg);   // versions this job adds (tile columns it covered)

@@ -10,7 +10,10 @@ SURVEY.md section 8(f) row 2 / PAPER.md:203 ("extend the library to distributed 
     received so far to the column it factors next, so per owned column there is one long contraction (efficient) and
     P - 1 short ones, and only a depth-one update plus the panel step sit between two consecutive broadcasts.
     Storage is replicated (every rank ends with the whole factor, which the prediction needs anyway: SURVEY.md 8(e));
-    the trailing-update WORK is what is divided.
+    the trailing-update WORK is what is divided.  Two transports for the panel: an NCCL broadcast of the packed tiles
+    after the panel step, or -- ``peers`` set -- the FUSED one: gp_mixed_panel_bcast stores every finished block straight
+    into the other ranks' copies of the tile array over NVLink peer memory while the panel step runs, and the
+    "broadcast" that follows is only a barrier (``exchange_peer_pointers`` sets the mapping up with CUDA IPC).
   * ``ShardedPredictor``: the prediction sharded by test-point tile rows: each rank
     solves V for its own test points, V^T is all-gathered once, each rank forms its block rows of Sigma.
 
@@ -73,6 +76,7 @@ class MixedCholeskyRank:
     rank: int
     world: int
     sched_width: int = 0
+    peers: tuple = ()          # device addresses of the other ranks' KL as seen from this GPU: the fused panel broadcast
 
     def __post_init__(self):
         self.M = self.n // self.tile
@@ -98,17 +102,25 @@ class MixedCholeskyRank:
         if kind == "update":
             gp.gp_mixed_update_column(self.KL, self.n, self.tile, op[1], op[2], op[3], self.work)
         elif kind == "panel":
-            gp.gp_mixed_panel(self.KL, self.n, self.tile, op[1], self.sched_width, self.info, self.work)
+            if self.peers:
+                gp.gp_mixed_panel_bcast(self.KL, self.n, self.tile, op[1], self.sched_width, self.info, self.work, self.peers)
+            else:
+                gp.gp_mixed_panel(self.KL, self.n, self.tile, op[1], self.sched_width, self.info, self.work)
         elif kind == "slice":
             gp.gp_mixed_slice_column(self.KL, self.n, self.tile, op[1], self.work)
         else:
             raise ValueError(op)
 
     def run(self, group=None) -> None:
-        """Execute the plan with NCCL broadcasts (one process per GPU)."""
+        """Execute the plan (one process per GPU): NCCL broadcasts of the packed panels, or, with `peers` set, the fused
+        transport: the owner's panel step has already written the panel into every copy, the broadcast is a barrier."""
         import torch.distributed as dist
         for op in self.ops:
-            if op[0] == "bcast":
+            if op[0] == "bcast" and self.peers:
+                if op[2] == self.rank:
+                    torch.cuda.current_stream().synchronize()        # the peer stores are complete when the panel step is
+                dist.barrier(group=group)
+            elif op[0] == "bcast":
                 J, root = op[1], op[2]
                 buf = self.pack_panel(J) if root == self.rank else torch.empty(self.M - J, self.tile * self.tile, dtype=torch.float64,
                                                                                device=self.KL.device)
@@ -132,15 +144,49 @@ def run_lockstep(states) -> None:
                 cursors[r] += 1
             assert st.ops[cursors[r]][1] == J
         root = states[0].ops[cursors[0]][2]
-        buf = states[root].pack_panel(J)
-        for r, st in enumerate(states):
-            if r != root:
-                st.unpack_panel(J, buf.clone())
+        if states[root].peers:
+            torch.cuda.current_stream().synchronize()     # fused transport: the panel step wrote every copy; this is the barrier
+        else:
+            buf = states[root].pack_panel(J)
+            for r, st in enumerate(states):
+                if r != root:
+                    st.unpack_panel(J, buf.clone())
+        for r in range(len(states)):
             cursors[r] += 1
     for r, st in enumerate(states):
         while cursors[r] < len(st.ops):
             st.compute(st.ops[cursors[r]])
             cursors[r] += 1
+
+
+def exchange_peer_pointers(KL: torch.Tensor, group=None):
+    """Addresses of the other ranks' `KL` as seen from this rank's GPU, in rank order without this rank: the `peers` of a
+    MixedCholeskyRank.  Every rank shares its tensor through CUDA IPC (torch.multiprocessing's reduction of a CUDA tensor:
+    cudaIpcGetMemHandle of its allocation + offset), the handles travel with all_gather_object, each rank opens the
+    others' (cudaIpcOpenMemHandle) and enables peer access to their devices.  Returns (addresses, keepalive): keep
+    `keepalive` referenced while the addresses are in use.  All GPUs of the node must be visible to every process.
+    UNVERIFIED ON MULTI-GPU HARDWARE (no such box was reachable): the one-GPU test covers the consumer of the addresses,
+    not this set-up."""
+    import ctypes
+    import torch.distributed as dist
+    from torch.multiprocessing.reductions import reduce_tensor
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    rebuild, args = reduce_tensor(KL)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, (rebuild, args), group=group)
+    cudart = ctypes.CDLL("libcudart.so")
+    views, addrs = [], []
+    for r, (fn, a) in enumerate(gathered):
+        if r == rank:
+            continue
+        t = fn(*a)                                   # a tensor on the owner's device, backed by the IPC mapping
+        if t.device != KL.device:
+            rc = cudart.cudaDeviceEnablePeerAccess(ctypes.c_int(t.device.index), ctypes.c_uint(0))
+            if rc not in (0, 704):                   # cudaSuccess, cudaErrorPeerAccessAlreadyEnabled
+                raise RuntimeError(f"cudaDeviceEnablePeerAccess({t.device.index}) failed: {rc}")
+        views.append(t)
+        addrs.append(int(t.data_ptr()))
+    return tuple(addrs), views
 
 
 # ------------------------------------------------------------------------------------------------

@@ -51,6 +51,40 @@ def test_block_cyclic_mixed_cholesky_in_lockstep_matches_oracle(gp, n, tile, wor
     assert torch.equal(states[0].KL, states[-1].KL) or relerr(_dense_L(gp, states[0].KL, n, tile), _dense_L(gp, states[-1].KL, n, tile)) == 0.0
 
 
+@pytest.mark.parametrize("n,tile,world", [(1024, 128, 2), (1536, 256, 3), (2048, 256, 8)])
+def test_block_cyclic_with_the_fused_panel_broadcast_matches_oracle_and_the_copy_transport(gp, n, tile, world):
+    """gp_mixed_panel_bcast: the owner's panel step stores every finished block into the other ranks' copies of the tile
+    array (here: other buffers of the same GPU standing in for NVLink peer memory), the broadcast is only a barrier.  Every
+    rank must end with the oracle's factor, bit-identical in its lower part to what the copy transport gives."""
+    from paper_2602_19683_b200 import multi_gpu as mg
+    D = 8
+    X, y = nfir.nfir_features(5 + world, n, D)
+    K = oracle.assemble(X, X, oracle.Hyper(), True)
+    Lo = oracle.cholesky(K)
+    ntiles = (n // tile) * (n // tile + 1) // 2
+    K0 = torch.empty(ntiles * tile * tile, dtype=torch.float64, device="cuda")
+    dX = torch.from_numpy(X).cuda()
+    gp.gp_assemble_tiles(dX, dX, gp.Hyper(), tile, gp.GP_SYM_LOWER, K0)
+    bufs = [K0.clone() for _ in range(world)]
+    states = [mg.MixedCholeskyRank(n, tile, bufs[r], torch.zeros(1, dtype=torch.int32, device="cuda"), r, world,
+                                   peers=tuple(int(bufs[q].data_ptr()) for q in range(world) if q != r)) for r in range(world)]
+    mg.run_lockstep(states)
+    torch.cuda.synchronize()
+    ref = [mg.MixedCholeskyRank(n, tile, K0.clone(), torch.zeros(1, dtype=torch.int32, device="cuda"), r, world) for r in range(world)]
+    mg.run_lockstep(ref)
+    torch.cuda.synchronize()
+    L_ref = _dense_L(gp, ref[0].KL, n, tile)
+    for r, st in enumerate(states):
+        assert int(st.info.item()) == 0
+        L = _dense_L(gp, st.KL, n, tile)
+        assert relerr(L, Lo) <= 1e-10, r
+        assert np.array_equal(L, L_ref), r
+    with pytest.raises(gp.GpError):                            # a peer must be another buffer
+        gp.gp_mixed_panel_bcast(bufs[0], n, tile, 0, 0, states[0].info, states[0].work, [int(bufs[0].data_ptr())])
+    with pytest.raises(gp.GpError):
+        gp.gp_mixed_panel_bcast(bufs[0], n, tile, 0, 0, states[0].info, states[0].work, [int(b.data_ptr()) for b in bufs] * 2)
+
+
 @pytest.mark.parametrize("n,m,D,tile,world", [(1024, 512, 8, 128, 2), (1024, 384, 8, 128, 2), (768, 768, 5, 256, 3), (16384 // 8, 1024, 8, 256, 4)])
 def test_sharded_prediction_in_lockstep_matches_oracle(gp, n, m, D, tile, world):
     from paper_2602_19683_b200 import multi_gpu as mg

@@ -149,6 +149,58 @@ def _gloo_worker(rank, world, port, out):
     np.save(f"{out}.{rank}.npy", np.array([err] + [x for ab in rows for x in ab]))
 
 
+def _gloo_worker_fused(rank, world, port, out, bufs):
+    """The fused transport on the CPU: every rank's tile array lives in shared memory (standing in for NVLink peer memory),
+    the owner of a panel writes the finished tiles into EVERY copy (what gp_mixed_panel_bcast does block by block), and the
+    "broadcast" is a barrier."""
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from paper_2602_19683_b200 import multi_gpu as mg
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    K, Lo = _problem()
+    st = _NumpyRank(K, 32, rank, world, mg)
+    index = {}
+    for I in range(st.M):
+        for J in range(I + 1):
+            index[(I, J)] = I * (I + 1) // 2 + J
+    views = [b.numpy() for b in bufs]                        # [ntiles, 32, 32] per rank
+    for key, k in index.items():                             # this rank's tiles move into its shared array
+        views[rank][k] = st.T[key]
+        st.T[key] = views[rank][k]
+    dist.barrier()
+    for op in st.ops:
+        if op[0] == "bcast":
+            dist.barrier()                                   # the owner's stores are complete: nothing to copy
+        elif op[0] == "panel":
+            st.compute(op)                                   # (results are assigned as new arrays ...)
+            J = op[1]
+            for I in range(J, st.M):
+                k = index[(I, J)]
+                for v in views:                              # ... and stored into every copy, the own one included
+                    v[k] = st.T[(I, J)]
+                st.T[(I, J)] = views[rank][k]
+        else:
+            st.compute(op)
+    err = float(np.linalg.norm(st.dense() - Lo) / np.linalg.norm(Lo))
+    dist.barrier()
+    dist.destroy_process_group()
+    np.save(f"{out}.{rank}.npy", np.array([err]))
+
+
+def test_block_cyclic_plan_with_the_fused_transport_over_shared_memory(tmp_path):
+    torch = pytest.importorskip("torch")
+    import torch.multiprocessing as mp
+    out = str(tmp_path / "f")
+    M = 256 // 32
+    bufs = [torch.zeros(M * (M + 1) // 2, 32, 32, dtype=torch.float64).share_memory_() for _ in range(2)]
+    mp.spawn(_gloo_worker_fused, args=(2, 29633, out, bufs), nprocs=2, join=True)
+    r = [np.load(f"{out}.{k}.npy") for k in range(2)]
+    assert r[0][0] <= 1e-12 and r[1][0] <= 1e-12
+
+
 def test_block_cyclic_plan_with_gloo_broadcasts(tmp_path):
     torch = pytest.importorskip("torch")
     import torch.multiprocessing as mp

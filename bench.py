@@ -66,6 +66,9 @@ def _parse():
                          "block-cyclic: ONE factorisation, tile columns distributed over the ranks, panels broadcast (NCCL), strong "
                          "scaling (SURVEY 8(f) row 2). shard-predict: replicated factor, prediction sharded by test-point tile rows "
                          "with one all-gather of V^T, strong scaling (SURVEY 8(e)). The last two are unmeasured on hardware.")
+    ap.add_argument("--fused-bcast", action="store_true",
+                    help="--mode block-cyclic: the panel step writes the panel into the other ranks' memory (gp_mixed_panel_bcast over CUDA IPC "
+                         "peer mappings) instead of an NCCL broadcast after it; unverified on multi-GPU hardware")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--cusolver-ref", action="store_true")
     ap.add_argument("--ozaki-probe", action="store_true", help="bounds of the emulated contraction (measurement support, one JSON line)")
@@ -442,7 +445,10 @@ def run_distributed(args):
 
     times = []
     if args.mode == "block-cyclic":
-        st = mg.MixedCholeskyRank(n, tile, pipe.KL, pipe.info, rank, world, args.width)
+        peers, keep = (), None
+        if world > 1 and args.fused_bcast:      # panels stored straight into the other ranks' copies (NVLink peer memory)
+            peers, keep = mg.exchange_peer_pointers(pipe.KL)
+        st = mg.MixedCholeskyRank(n, tile, pipe.KL, pipe.info, rank, world, args.width, peers)
         for it in range(args.warmup + args.steps):
             pipe.assemble(dX)
             st.reset()
@@ -457,7 +463,9 @@ def run_distributed(args):
             barrier()
             if it >= args.warmup:
                 times.append(a.elapsed_time(b))
-        what = "Cholesky, tile columns block-cyclic over the ranks, FP64 panels broadcast, int8-emulated trailing updates"
+        what = ("Cholesky, tile columns block-cyclic over the ranks, FP64 panels " +
+                ("stored into every rank's copy by the panel step itself (fused broadcast over peer memory)" if peers else "broadcast with NCCL") +
+                ", int8-emulated trailing updates")
     else:
         pipe.assemble(dX); pipe.cholesky(); pipe.solve(dY)   # replicated factor (not timed)
         sp = mg.ShardedPredictor(n, m, D, tile, h, rank, world, args.width)

@@ -641,6 +641,20 @@ def run_b200(args):
     barrier()
     e2e_ms = a.elapsed_time(b)
     del ws
+    # the same host-to-host call with the int8-emulated factorisation and covariance (reported beside the headline)
+    if "cholesky_mixed_int8_emulated" in next_rows and m <= 65536:
+        torch.cuda.empty_cache()
+        wsm = torch.empty(gp.gp_pipeline_mixed_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
+        gp.gp_pipeline_host(hX, hY, hXs, h, tile, args.width, hMean, hSigma, None, wsm, mixed=True)
+        reps = max(1, min(args.steps, 3))
+        a2, b2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a2.record()
+        for _ in range(reps):
+            info_m = gp.gp_pipeline_host(hX, hY, hXs, h, tile, args.width, hMean, hSigma, None, wsm, mixed=True)
+        b2.record(); torch.cuda.synchronize()
+        next_rows["pipeline_host_mixed_int8_emulated"] = {"ms": a2.elapsed_time(b2) / reps, "fp64_path_ms": e2e_ms / args.steps, "info": info_m,
+                                                          "call": "gp_pipeline_host_mixed (pinned host buffers; a1-a12 + copies)"}
+        del wsm
 
     t = reduce_max_over_ranks([phase[nm] for nm in names] + [total_ms, e2e_ms], device="cuda")
     phase = {nm: t[i] / args.steps for i, nm in enumerate(names)}

@@ -180,6 +180,13 @@ int gp_pipeline_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* b
 int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D,
                      gp_hyper h, int tile, int sched_width, double* hMean, double* hSigma, double* hAlpha,
                      int* h_info, void* dWork, size_t work_bytes, void* stream);
+/* The same call with the O(n^3) contractions emulated on the int8 tensor cores: gp_cholesky_tiled_mixed
+ * and gp_predict_full_cov_mixed in place of gp_cholesky_tiled and gp_predict_full_cov; same arguments, same outputs within
+ * the oracle tolerances, tile % 128 == 0, and a larger scratch (gp_pipeline_mixed_workspace_bytes: the digit planes). */
+int gp_pipeline_mixed_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* bytes);
+int gp_pipeline_host_mixed(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D,
+                           gp_hyper h, int tile, int sched_width, double* hMean, double* hSigma, double* hAlpha,
+                           int* h_info, void* dWork, size_t work_bytes, void* stream);
 
 /* FP64 peak microbenchmark launch (measurement support; north_star: "FP64 peak also measured by a
  * microbenchmark").  Enqueues one launch of independent register-resident chains on every SM:

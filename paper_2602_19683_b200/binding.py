@@ -21,7 +21,7 @@ ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA":
 
 EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
-           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
+           "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_pipeline_mixed_workspace_bytes", "gp_pipeline_host_mixed", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
@@ -87,6 +87,8 @@ def load() -> ctypes.CDLL:
     lib.gp_strerror.argtypes = [ci]
     lib.gp_pipeline_workspace_bytes.argtypes = [i64, i64, ci, ci, psz]
     lib.gp_pipeline_host.argtypes = [vp, vp, vp, i64, i64, ci, gp_hyper, ci, ci, vp, vp, vp, vp, vp, sz, vp]
+    lib.gp_pipeline_host_mixed.argtypes = [vp, vp, vp, i64, i64, ci, gp_hyper, ci, ci, vp, vp, vp, vp, vp, sz, vp]
+    lib.gp_pipeline_mixed_workspace_bytes.argtypes = [i64, i64, ci, ci, psz]
     lib.gp_schedule_selfcheck.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_schedule_selfcheck_variance.argtypes = [i64, i64, ci, ci, ctypes.POINTER(ctypes.c_double)]
     lib.gp_exec_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ci, vp]
@@ -244,6 +246,12 @@ def gp_pipeline_workspace_bytes(n: int, m: int, D: int, tile: int) -> int:
     return int(b.value)
 
 
+def gp_pipeline_mixed_workspace_bytes(n: int, m: int, D: int, tile: int) -> int:
+    b = ctypes.c_size_t(0)
+    _check(load().gp_pipeline_mixed_workspace_bytes(n, m, D, tile, ctypes.byref(b)), "gp_pipeline_mixed_workspace_bytes")
+    return int(b.value)
+
+
 def _hptr(t: torch.Tensor | None, dtype=torch.float64):
     if t is None:
         return None
@@ -253,12 +261,14 @@ def _hptr(t: torch.Tensor | None, dtype=torch.float64):
 
 
 def gp_pipeline_host(hX: torch.Tensor, hY: torch.Tensor, hXs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
-                     hMean: torch.Tensor, hSigma: torch.Tensor | None, hAlpha: torch.Tensor | None, work: torch.Tensor) -> int:
-    """HOST tensors in, HOST tensors out (pinned recommended); `work` is device scratch. Returns info."""
+                     hMean: torch.Tensor, hSigma: torch.Tensor | None, hAlpha: torch.Tensor | None, work: torch.Tensor, mixed: bool = False) -> int:
+    """HOST tensors in, HOST tensors out (pinned recommended); `work` is device scratch. Returns info.  mixed: the int8-emulated
+    factorisation and covariance (gp_pipeline_host_mixed; `work` from gp_pipeline_mixed_workspace_bytes)."""
     n, D = hX.shape
     m = hXs.shape[0]
     info = ctypes.c_int(0)
-    _check(load().gp_pipeline_host(_hptr(hX), _hptr(hY), _hptr(hXs), n, m, D, h.c(), tile, sched_width, _hptr(hMean),
+    fn = load().gp_pipeline_host_mixed if mixed else load().gp_pipeline_host
+    _check(fn(_hptr(hX), _hptr(hY), _hptr(hXs), n, m, D, h.c(), tile, sched_width, _hptr(hMean),
                                    _hptr(hSigma), _hptr(hAlpha), ctypes.byref(info), _ptr(work, torch.uint8), work.numel(),
                                    _stream()), "gp_pipeline_host")
     return int(info.value)

@@ -711,10 +711,14 @@ void gp_release_cached_schedules(void) {
 // ---- whole pipeline on host buffers -----------------------------------------------------------
 namespace {
 struct PipeWs { size_t X, y, Xs, KL, alpha, beta, mean, Sigma, info, scratch, scratch_bytes, total; };
-int pipe_ws(int64_t n, int64_t m, int D, int tile, PipeWs* w) {
+int pipe_ws(int64_t n, int64_t m, int D, int tile, PipeWs* w, bool mixed = false) {
     size_t c = 0, s = 0, f = 0;
     int rc = gp_workspace_bytes(n, m, D, tile, &c, &s, &f);
     if (rc != GP_OK) return rc;
+    if (mixed) {        // the emulated path: its scratch (digit planes of L and V^T) replaces the executor's
+        if ((rc = gp_mixed_workspace_bytes(n, tile, &c)) != GP_OK) return rc;
+        if (m > 0 && (rc = gp_mixed_predict_workspace_bytes(n, m, tile, &f)) != GP_OK) return rc;
+    }
     const size_t M = (size_t)(n / tile);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
@@ -745,14 +749,23 @@ int gp_pipeline_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* b
     return GP_OK;
 }
 
-int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D, gp_hyper h, int tile,
-                     int sched_width, double* hMean, double* hSigma, double* hAlpha, int* h_info, void* dWork, size_t work_bytes,
-                     void* stream) {
+int gp_pipeline_mixed_workspace_bytes(int64_t n, int64_t m, int D, int tile, size_t* bytes) {
+    if (!bytes) return GP_ERR_NULL;
+    PipeWs w;
+    int rc = pipe_ws(n, m, D, tile, &w, true);
+    if (rc != GP_OK) return rc;
+    *bytes = w.total;
+    return GP_OK;
+}
+
+static int pipeline_host_impl(bool mixed, const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D, gp_hyper h, int tile,
+                              int sched_width, double* hMean, double* hSigma, double* hAlpha, int* h_info, void* dWork, size_t work_bytes,
+                              void* stream) {
     if (!hX || !hY || !hXs || !hMean || !h_info || !dWork) return GP_ERR_NULL;
     if (m <= 0) return GP_ERR_SIZE;
     if (!hyper_ok(h)) return GP_ERR_HYPER;
     PipeWs w;
-    int rc = pipe_ws(n, m, D, tile, &w);
+    int rc = pipe_ws(n, m, D, tile, &w, mixed);
     if (rc != GP_OK) return rc;
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
@@ -766,11 +779,15 @@ int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int6
     if (cudaMemcpyAsync(dY, hY, (size_t)n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return GP_ERR_CUDA;
     if (cudaMemcpyAsync(dXs, hXs, (size_t)m * D * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return GP_ERR_CUDA;
     if ((rc = gp_assemble_tiles(dX, n, dX, n, D, h, tile, GP_SYM_LOWER, dKL, stream)) != GP_OK) return rc;
-    if ((rc = gp_cholesky_tiled(dKL, n, tile, sched_width, d_info, scratch, w.scratch_bytes, stream)) != GP_OK) return rc;
+    rc = mixed ? gp_cholesky_tiled_mixed(dKL, n, tile, sched_width, d_info, scratch, w.scratch_bytes, stream)
+               : gp_cholesky_tiled(dKL, n, tile, sched_width, d_info, scratch, w.scratch_bytes, stream);
+    if (rc != GP_OK) return rc;
     if ((rc = gp_solve(dKL, n, tile, dY, dAlpha, dBeta, scratch, w.scratch_bytes, stream)) != GP_OK) return rc;
     if ((rc = gp_predict_mean(dX, n, D, dAlpha, dXs, m, h, dMean, stream)) != GP_OK) return rc;
     if (hSigma) {
-        if ((rc = gp_predict_full_cov(dKL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, scratch, w.scratch_bytes, stream)) != GP_OK)
+        rc = mixed ? gp_predict_full_cov_mixed(dKL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, scratch, w.scratch_bytes, stream)
+                   : gp_predict_full_cov(dKL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, scratch, w.scratch_bytes, stream);
+        if (rc != GP_OK)
             return rc;
         if (cudaMemcpyAsync(hSigma, dSigma, (size_t)m * m * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
     }
@@ -778,6 +795,18 @@ int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int6
     if (hAlpha && cudaMemcpyAsync(hAlpha, dAlpha, (size_t)n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
     if (cudaMemcpyAsync(h_info, d_info, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return GP_ERR_CUDA;
     return cudaStreamSynchronize(st) == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+int gp_pipeline_host(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D, gp_hyper h, int tile,
+                     int sched_width, double* hMean, double* hSigma, double* hAlpha, int* h_info, void* dWork, size_t work_bytes,
+                     void* stream) {
+    return pipeline_host_impl(false, hX, hY, hXs, n, m, D, h, tile, sched_width, hMean, hSigma, hAlpha, h_info, dWork, work_bytes, stream);
+}
+
+int gp_pipeline_host_mixed(const double* hX, const double* hY, const double* hXs, int64_t n, int64_t m, int D, gp_hyper h, int tile,
+                           int sched_width, double* hMean, double* hSigma, double* hAlpha, int* h_info, void* dWork, size_t work_bytes,
+                           void* stream) {
+    return pipeline_host_impl(true, hX, hY, hXs, n, m, D, h, tile, sched_width, hMean, hSigma, hAlpha, h_info, dWork, work_bytes, stream);
 }
 
 int gp_fp64_peak_launch(int mode, int iters, double* d_sink, double* flops, void* stream) {

@@ -229,6 +229,29 @@ def test_host_buffer_pipeline_matches_oracle(gp):
     assert e.value.code == gp.ERR["WORKSPACE"]
 
 
+def test_host_buffer_pipeline_with_the_emulated_contractions_matches_oracle(gp):
+    """gp_pipeline_host_mixed: the same call with the factorisation and the covariance on the int8-emulated contraction."""
+    n, m, D, tile = 1536, 512, 8, 256
+    X, y = nfir.nfir_features(31, n, D)
+    Xs, _ = nfir.nfir_features(32, m, D, with_targets=False)
+    h = oracle.Hyper()
+    p = oracle.predict(X, y, Xs, h)
+    hX, hY, hXs = (torch.from_numpy(a).pin_memory() for a in (X, y, Xs))
+    hMean = torch.empty(m, dtype=torch.float64).pin_memory()
+    hSigma = torch.empty(m, m, dtype=torch.float64).pin_memory()
+    hAlpha = torch.empty(n, dtype=torch.float64).pin_memory()
+    ws = torch.empty(gp.gp_pipeline_mixed_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
+    info = gp.gp_pipeline_host(hX, hY, hXs, gp.Hyper(), tile, 0, hMean, hSigma, hAlpha, ws, mixed=True)
+    assert info == 0
+    assert relerr(hAlpha.numpy(), p.alpha) <= TOL_ALPHA
+    assert relerr(hMean.numpy(), p.mean) <= TOL_MEAN
+    assert relerr(hSigma.numpy(), p.Sigma) <= TOL_SIGMA
+    small = torch.empty(gp.gp_pipeline_workspace_bytes(n, m, D, tile), dtype=torch.uint8, device="cuda")
+    with pytest.raises(gp.GpError) as e:
+        gp.gp_pipeline_host(hX, hY, hXs, gp.Hyper(), tile, 0, hMean, hSigma, None, small, mixed=True)
+    assert e.value.code == gp.ERR["WORKSPACE"]
+
+
 def test_fp64_peak_probe_launches(gp):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     for mode in (0, 1):

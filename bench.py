@@ -622,7 +622,18 @@ def run_b200(args):
                 "ms": statistics.median(tpx), "fp64_path_ms": phase_full_cov_ms,
                 "rel_diff_to_fp64_sigma": float((pipe.Sigma - S64).norm() / S64.norm()),
                 "what": "gp_predict_full_cov_mixed: V^T solve and W = V^T V as split-operand int8 products, TRSM with the diagonal tiles in FP64"}
-            del S64, pwork
+            varm = torch.empty(m, dtype=torch.float64, device="cuda")
+            tvx = []
+            for r in range(3):
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                e[0].record(); gp.gp_predict_variance_mixed(pipe.KL, dX, dXs, h, tile, args.width, varm, pwork); e[1].record()
+                torch.cuda.synchronize()
+                if r > 0:
+                    tvx.append(e[0].elapsed_time(e[1]))
+            next_rows["predict_variance_mixed_int8_emulated"] = {
+                "ms": statistics.median(tvx), "fp64_path_ms": next_rows["predict_variance_ms"],
+                "max_abs_diff_to_diag_of_fp64_sigma": float((varm - torch.diagonal(S64)).abs().max())}
+            del S64, pwork, varm
     torch.cuda.empty_cache()
 
     # end to end through the host-buffer C-ABI call: H2D of X, y, X^ and D2H of mean, Sigma inside

@@ -299,10 +299,14 @@ int gp_mixed_panel_bcast(double* dKL, int64_t n, int tile, int J, int sched_widt
  * TRSM with the diagonal tile on the executor, then its digit planes), and W = V^T (V^T)^T in ONE emulated contraction of
  * depth n over the lower triangle of Sigma, mirrored.  Arguments as gp_predict_full_cov; additionally tile % 128 == 0,
  * n / tile <= 60, n <= 65536, m <= 65536.  dWork: gp_mixed_predict_workspace_bytes() (V^T and the digit planes of L and
- * of V^T: 8 (m n + n^2 + m n) bytes). */
+ * of V^T: 8 m n + 7 (n^2 + m n) bytes). */
 int gp_mixed_predict_workspace_bytes(int64_t n, int64_t m, int tile, size_t* bytes);
 int gp_predict_full_cov_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
                               int tile, int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream);
+/* Variances only on the emulated contraction (SURVEY.md 8(f) rows 1 and 3 together): the V^T solve of
+ * gp_predict_full_cov_mixed without W, then var_a = v - sum_i V_ia^2 as gp_predict_variance.  dVar [m]; same scratch. */
+int gp_predict_variance_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
+                              int tile, int sched_width, double* dVar, void* dWork, size_t work_bytes, void* stream);
 
 /* Host-only replay check of the panel schedule of step J (returns the number of work items, or a negative GP_ERR_*). */
 int gp_panel_schedule_selfcheck(int64_t n, int tile, int J);

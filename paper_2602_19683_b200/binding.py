@@ -25,7 +25,7 @@ EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mea
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
            "gp_schedule_selfcheck_variance", "gp_prepare", "gp_schedule_fingerprint",
            "gp_set_schedule_granularity", "gp_schedule_granularity", "gp_block_size_for", "gp_set_block_edge",
-           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_mixed_panel_bcast", "gp_int8_mma_peak_launch", "gp_ozaki_probe_launch", "gp_ozaki_probe_stamps", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
+           "gp_ozaki_planes", "gp_ozaki_digit_bits", "gp_mixed_panel_bcast", "gp_predict_variance_mixed", "gp_int8_mma_peak_launch", "gp_ozaki_probe_launch", "gp_ozaki_probe_stamps", "gp_ozaki_plane_bytes", "gp_ozaki_slice", "gp_ozaki_contract",
            "gp_mixed_workspace_bytes", "gp_cholesky_tiled_mixed", "gp_panel_schedule_selfcheck",
            "gp_mixed_begin", "gp_mixed_update_column", "gp_mixed_panel", "gp_mixed_slice_column",
            "gp_predict_vt", "gp_cov_rows_workspace_bytes", "gp_predict_cov_rows", "gp_set_ozaki_tile_n",
@@ -111,6 +111,7 @@ def load() -> ctypes.CDLL:
     lib.gp_set_ozaki_tile_n.argtypes = [ci]
     lib.gp_mixed_predict_workspace_bytes.argtypes = [i64, i64, ci, psz]
     lib.gp_predict_full_cov_mixed.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
+    lib.gp_predict_variance_mixed.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_ozaki_slice.argtypes = [vp, i64, i64, i64, ctypes.c_double, vp, vp, vp]
     lib.gp_ozaki_contract.argtypes = [vp, i64, vp, i64, i64, ctypes.c_double, ctypes.c_double, vp, i64, vp]
     lib.gp_block_size_for.argtypes = [i64, ci]
@@ -207,6 +208,15 @@ def gp_predict_variance(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: H
     m = Xs.shape[0]
     _check(load().gp_predict_variance(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(var),
                                       _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_variance")
+
+
+def gp_predict_variance_mixed(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int,
+                              var: torch.Tensor, work: torch.Tensor) -> None:
+    """gp_predict_variance with the V^T solve on the int8-emulated contraction (work: gp_mixed_predict_workspace_bytes)."""
+    n, D = X.shape
+    m = Xs.shape[0]
+    _check(load().gp_predict_variance_mixed(_ptr(L), _ptr(X), n, D, _ptr(Xs), m, h.c(), tile, sched_width, _ptr(var),
+                                            _ptr(work, torch.uint8), work.numel(), _stream()), "gp_predict_variance_mixed")
 
 
 def gp_predict_vt(L: torch.Tensor, X: torch.Tensor, Xs: torch.Tensor, h: Hyper, tile: int, sched_width: int, Vt: torch.Tensor,

@@ -1280,9 +1280,11 @@ extern "C" int gp_mixed_predict_workspace_bytes(int64_t n, int64_t m, int tile, 
     return GP_OK;
 }
 
-extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
-                                         int tile, int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
-    if (!dL || !dX || !dXs || !dSigma || !dWork) return GP_ERR_NULL;
+namespace {
+// dSigma: full covariance (V^T solve + W on the emulated contraction); dVar (dSigma null): variances only, the V^T solve alone
+int predict_mixed_impl(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h, int tile, int sched_width,
+                       double* dSigma, double* dVar, void* dWork, size_t work_bytes, void* stream) {
+    if (!dL || !dX || !dXs || (!dSigma && !dVar) || !dWork) return GP_ERR_NULL;
     int rc = mixed_ok(n, tile);
     if (rc != GP_OK) return rc;
     if (m <= 0 || m > 65536 || D <= 0) return GP_ERR_SIZE;
@@ -1306,7 +1308,7 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
     if (cudaMemsetAsync(scale, 0, 256, st) != cudaSuccess) return GP_ERR_CUDA;
     // a9: K_{X^,X} straight into V^T, the prior K_{X^,X^} straight into Sigma (as gp_predict_full_cov)
     if ((rc = launch_assemble(dXs, m, dX, n, D, hd, tile, 0, Vt, st)) != GP_OK) return rc;
-    {
+    if (dSigma) {
         const int sb = (int)((m + kAsmBlk - 1) / kAsmBlk);
         const size_t smem = 2 * (size_t)kAsmMaxD * kAsmBlk * sizeof(double);
         assemble_tiles_kernel<<<(unsigned)(sb * sb), 256, smem, st>>>(dXs, dXs, D, hd, (int)m, 1, 0, dSigma);
@@ -1367,11 +1369,16 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
         row_items_set_column_kernel<<<(NBm + 255) / 256, 256, 0, st>>>((uint4*)items, NBm, (unsigned)(P * nbt));
         p.ticket = (unsigned int*)(ws + w.ticket) + P;
         if ((rc = launch_exec<128>(p, mp, workers_for(sched_width), st)) != GP_OK) return rc;
-        {
+        if (dSigma || P + 1 < M) {              // the last column's planes only feed W
             const int64_t total = m * (tile / 4);
             const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);
             oz::slice_general_column_kernel<<<grid, 256, 0, st>>>(Vt, m, n, tile, P, scale + 1, planesV);
         }
+    }
+    if (!dSigma) {
+        // var_a = k(x^_a, x^_a) - sum_i V_ia^2, as gp_predict_variance
+        posterior_var_kernel<<<(unsigned)((m + 7) / 8), 256, 0, st>>>(Vt, m, n, tile, hd.vertical, dVar);
+        return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
     }
     {   // a12: Sigma -= V^T (V^T)^T over the lower triangle, one emulated contraction of depth n; then the mirror
         oz::OzParams q;
@@ -1388,6 +1395,19 @@ extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int
     dim3 mg((unsigned)(m / 32), (unsigned)(m / 32));
     mirror_lower_kernel<<<mg, dim3(32, 8), 0, st>>>(dSigma, m);
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+}  // namespace
+
+extern "C" int gp_predict_full_cov_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
+                                         int tile, int sched_width, double* dSigma, void* dWork, size_t work_bytes, void* stream) {
+    if (!dSigma) return GP_ERR_NULL;
+    return predict_mixed_impl(dL, dX, n, D, dXs, m, h, tile, sched_width, dSigma, nullptr, dWork, work_bytes, stream);
+}
+
+extern "C" int gp_predict_variance_mixed(const double* dL, const double* dX, int64_t n, int D, const double* dXs, int64_t m, gp_hyper h,
+                                         int tile, int sched_width, double* dVar, void* dWork, size_t work_bytes, void* stream) {
+    if (!dVar) return GP_ERR_NULL;
+    return predict_mixed_impl(dL, dX, n, D, dXs, m, h, tile, sched_width, nullptr, dVar, dWork, work_bytes, stream);
 }
 
 extern "C" int gp_panel_schedule_selfcheck(int64_t n, int tile, int J) {

@@ -169,6 +169,13 @@ def test_mixed_prediction_matches_oracle(gp, n, m, D, tile):
     assert np.array_equal(S, S.T)
     d = np.diag(S)
     assert d.min() >= 0.0 and d.max() <= h.vertical
+    # variances only (8(f) row 1 on the emulated V^T solve): the oracle's posterior variances
+    var = torch.empty(m, dtype=torch.float64, device="cuda")
+    gp.gp_predict_variance_mixed(pipe.KL, dX, dXs, hg, tile, 0, var, work)
+    torch.cuda.synchronize()
+    want = oracle.posterior_var(p.V, h.vertical * np.ones(m))
+    assert relerr(var.cpu().numpy(), want) <= 1e-9
+    np.testing.assert_allclose(var.cpu().numpy(), np.diag(p.Sigma), rtol=0, atol=1e-9 * h.vertical)
 
 
 # ---------------------------------------------------------------- measurement support

@@ -23,7 +23,8 @@ def gp():
 
 
 # (256, 512), (384, 1152) and (1280, 2048) take the 128 x 128 two-pass kernel, the others the 128 x 64 one (m or n not a multiple of 128)
-@pytest.mark.parametrize("m,n", [(128, 32), (256, 512), (640, 1056), (384, 1152), (1280, 2048)])
+# (1792, 256): 14 x 14 output tiles, more than the band height of the wide kernel's tile order (a band of 12 rows + one of 2)
+@pytest.mark.parametrize("m,n", [(128, 32), (256, 512), (640, 1056), (384, 1152), (1280, 2048), (1792, 256)])
 def test_emulated_contraction_matches_oracle_posterior_cov(gp, m, n):
     rng = np.random.default_rng(m + n)
     V = rng.uniform(-0.9, 0.9, size=(n, m))                     # |V| <= 1 as for V = L^-1 K_{X,X^} with v = 1
@@ -143,7 +144,8 @@ def test_mixed_cholesky_reports_a_non_positive_pivot(gp):
     assert int(info.item()) == 301
 
 
-@pytest.mark.parametrize("n,m,D,tile", [(512, 256, 8, 128), (1024, 512, 8, 256), (2048, 1024, 5, 512), (1536, 256, 8, 256)])
+# (1024, 2048, ...): Sigma has 16 x 16 output tiles: the banded tile order together with the lower-triangle selection
+@pytest.mark.parametrize("n,m,D,tile", [(512, 256, 8, 128), (1024, 512, 8, 256), (2048, 1024, 5, 512), (1536, 256, 8, 256), (1024, 2048, 8, 256)])
 def test_mixed_prediction_matches_oracle(gp, n, m, D, tile):
     """gp_predict_full_cov_mixed (V^T solve and W on the emulated contraction, TRSM with the diagonal tiles in FP64) on the
     factor of gp_cholesky_tiled_mixed: Sigma against the oracle at north_star's 1e-9, exactly symmetric."""
@@ -215,3 +217,24 @@ def test_probe_launch_without_a_switch_is_the_product_kernel(gp):
         assert len(t) == 8
     with pytest.raises(gp.GpError):
         gp.gp_ozaki_probe_launch(3, planes, planes, C2)
+
+
+def test_wide_kernel_is_bit_reproducible_over_many_runs(gp):
+    """Race hunt for the 128 x 128 two-pass kernel (ring slots retired by tcgen05.commit, tensor memory handed between the
+    passes, staging boxes reused behind bulk-group waits): 40 runs of a multi-tile, multi-wave product must give the same
+    bits (integer level sums and a fixed recombination order leave no room for run-to-run differences)."""
+    rng = np.random.default_rng(5)
+    m, k = 2304, 1408                      # 18 x 18 tiles (324 > 148 CTAs: two and a bit waves), 11 k-chunks
+    A = torch.from_numpy(rng.uniform(-0.9, 0.9, size=(m, k))).cuda()
+    planes = gp.gp_ozaki_slice(A, 2.0)
+    C0 = torch.from_numpy(rng.normal(size=(m, m))).cuda()
+    first = None
+    for _ in range(40):
+        C = C0.clone()
+        gp.gp_ozaki_contract(planes, planes, 2.0, 2.0, C)
+        torch.cuda.synchronize()
+        if first is None:
+            first = C
+            assert relerr(C.cpu().numpy(), (C0 - A @ A.T).cpu().numpy()) <= 1e-14
+        else:
+            assert torch.equal(C, first)

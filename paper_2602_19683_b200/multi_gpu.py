@@ -165,8 +165,8 @@ def exchange_peer_pointers(KL: torch.Tensor, group=None):
     cudaIpcGetMemHandle of its allocation + offset), the handles travel with all_gather_object, each rank opens the
     others' (cudaIpcOpenMemHandle) and enables peer access to their devices.  Returns (addresses, keepalive): keep
     `keepalive` referenced while the addresses are in use.  All GPUs of the node must be visible to every process.
-    UNVERIFIED ON MULTI-GPU HARDWARE (no such box was reachable): the one-GPU test covers the consumer of the addresses,
-    not this set-up."""
+    Verified between two processes on ONE GPU (tests/test_gpu_multi.py); across two physical GPUs (peer access over
+    NVLink) it is UNVERIFIED: no such box was reachable."""
     import ctypes
     import torch.distributed as dist
     from torch.multiprocessing.reductions import reduce_tensor

@@ -113,3 +113,61 @@ def test_sharded_prediction_in_lockstep_matches_oracle(gp, n, m, D, tile, world)
     Vt = torch.empty(m, n, dtype=torch.float64, device="cuda")
     gp.gp_tiles_to_dense(ranks[0].Vt_all, m, n, tile, False, Vt)
     assert relerr(Vt.cpu().numpy().T, p.V) <= 1e-9
+
+
+def _ipc_worker(rank, world, port, out):
+    import os
+    import sys
+    import torch.distributed as dist
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for q in (root, os.path.join(root, "tests")):
+        if q not in sys.path:
+            sys.path.insert(0, q)
+    from paper_2602_19683_b200 import binding as gpb, multi_gpu as mg
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    gpb.load()
+    n, tile, D = 1024, 128, 8
+    X, _ = nfir.nfir_features(7, n, D)
+    Lo = oracle.cholesky(oracle.assemble(X, X, oracle.Hyper(), True))
+    ntiles = (n // tile) * (n // tile + 1) // 2
+    KL = torch.empty(ntiles * tile * tile, dtype=torch.float64, device="cuda")
+    dX = torch.from_numpy(X).cuda()
+    gpb.gp_assemble_tiles(dX, dX, gpb.Hyper(), tile, gpb.GP_SYM_LOWER, KL)
+    torch.cuda.synchronize()
+    peers, keep = mg.exchange_peer_pointers(KL)              # CUDA IPC: the other process's tile array mapped into this one
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    st = mg.MixedCholeskyRank(n, tile, KL, info, rank, world, 0, peers)
+    torch.cuda.synchronize()
+    dist.barrier()
+    st.run()                                                 # fused transport: panels are stored into the peer, then a barrier
+    torch.cuda.synchronize()
+    dist.barrier()
+    dense = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    L = gpb.gp_tiles_to_dense(KL, n, n, tile, True, dense).cpu().numpy()
+    np.save(f"{out}.{rank}.npy", np.array([relerr(L, Lo), float(info.item())]))
+    dist.barrier()
+    del keep
+    dist.destroy_process_group()
+
+
+@pytest.mark.timeout(600)
+def test_fused_panel_broadcast_across_two_processes_over_cuda_ipc(gp, tmp_path):
+    """The one piece of the fused transport the lock-step emulation does not reach: multi_gpu.exchange_peer_pointers (CUDA
+    IPC handles through all_gather_object, cudaIpcOpenMemHandle) and MixedCholeskyRank.run() with barriers.  Two PROCESSES
+    share this one GPU (host-side gloo barriers only: no kernel waits on another); each must end with the oracle's factor,
+    half of whose panels arrived as stores from the other process.  Stands in for two GPUs over NVLink, which this box
+    does not have."""
+    import torch.multiprocessing as mp
+    out = str(tmp_path / "ipc")
+    try:
+        mp.spawn(_ipc_worker, args=(2, 29657, out), nprocs=2, join=True)
+    except Exception as e:                                   # a sandbox that forbids CUDA IPC between processes
+        if "ipc" in str(e).lower():
+            pytest.skip(f"CUDA IPC between processes is not available here: {str(e)[-200:]}")
+        raise
+    for r in range(2):
+        err, info = np.load(f"{out}.{r}.npy")
+        assert info == 0 and err <= 1e-10, (r, err, info)

@@ -1065,12 +1065,14 @@ extern "C" int gp_ozaki_contract(const int8_t* dAplanes, int64_t ma, const int8_
 namespace {
 struct MixedWs { size_t ticket, verL, invD, scale, planes, total; };
 MixedWs mixed_ws(int64_t n) {
-    const CholWs c = chol_ws(n, 128);
+    // panels run with 128-blocks or, when few block rows are left below the diagonal tile, with 64-blocks (mixed_panel_block):
+    // version counters for the finer grid, inverted diagonal blocks for the coarser one (n x 128 doubles covers n x 64)
+    const CholWs c = chol_ws(n, 64), c128 = chol_ws(n, 128);
     MixedWs w;
     w.ticket = c.ticket;
     w.verL = c.verL;
     w.invD = c.invD;
-    w.scale = align_up(c.total, 256);
+    w.scale = align_up(c.invD + (c128.total - c128.invD), 256);
     w.planes = align_up(w.scale + 256, 1024);
     w.total = w.planes + (size_t)oz::kPlanes * (size_t)n * (size_t)n;
     return w;
@@ -1116,15 +1118,24 @@ int mixed_ctx(int64_t n, int tile, void* dWork, size_t work_bytes, void* stream,
     c->st = (cudaStream_t)stream;
     return GP_OK;
 }
-int get_panel_schedule(int M, int nbt, int J, CachedSchedule* out) {
+// Block edge of the FP64 panel step of column J.  A panel is the chain of the diagonal tile (tile / b dependent POTRF -> solve ->
+// update steps: 86 us each with 128-blocks, 29 us with 64-blocks) and the solves of the block rows below it.  With many rows
+// the solves are the bulk and 128-blocks run them at the DMMA rate (64-blocks reach ~80 % of it); with few rows the chain is
+// all there is, and 64-blocks halve it: c3 panels J >= 18: 0.96 -> ~0.6 ms each.
+int mixed_panel_block(int M, int tile, int J) {
+    const int rows128 = (M - J - 1) * (tile / 128);
+    return rows128 <= 104 ? 64 : 128;
+}
+
+int get_panel_schedule(int M, int nbt, int J, int b, CachedSchedule* out) {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
     std::lock_guard<std::mutex> lk(g_mu);
-    auto key = std::make_tuple(dev, 16 + J, M, 0, nbt, 128);
+    auto key = std::make_tuple(dev, 16 + J, M, 0, nbt, b);
     auto it = g_cache.find(key);
     if (it != g_cache.end()) { *out = it->second; return GP_OK; }
     std::vector<SchedItem> items;
-    build_panel_schedule(M, nbt, J, sm_count(), items, 128);
+    build_panel_schedule(M, nbt, J, sm_count(), items, b);
     CachedSchedule cs;
     cs.nitems = (int)items.size();
     if (cudaMalloc(&cs.d_items, items.size() * sizeof(Item) + 16) != cudaSuccess) return GP_ERR_CUDA;
@@ -1185,8 +1196,10 @@ int mixed_panel_impl(double* dKL, int64_t n, int tile, int J, int sched_width, i
     int rc = mixed_ctx(n, tile, dWork, work_bytes, stream, &c);
     if (rc != GP_OK) return rc;
     if (J < 0 || J >= c.M) return GP_ERR_SIZE;
+    const int b = mixed_panel_block(c.M, tile, J);
+    const int nbt = tile / b, NB = (int)(n / b);
     CachedSchedule cs;
-    if ((rc = get_panel_schedule(c.M, c.nbt, J, &cs)) != GP_OK) return rc;
+    if ((rc = get_panel_schedule(c.M, nbt, J, b, &cs)) != GP_OK) return rc;
     ExecParams p;
     memset(&p, 0, sizeof(p));
     p.L = dKL;
@@ -1195,21 +1208,19 @@ int mixed_panel_impl(double* dKL, int64_t n, int tile, int J, int sched_width, i
     p.stats = (unsigned long long*)(c.ws + kStatsOff);
     p.d_info = d_info;
     p.t = tile;
-    p.nbt = c.nbt;
-    p.snbt = c.nbt;
-    p.NB = c.NB;
+    p.nbt = nbt;
+    p.snbt = nbt;
+    p.NB = NB;
     p.Mt = c.M;
     p.items = cs.d_items;
     p.nitems = cs.nitems;
     p.ticket = (unsigned int*)(c.ws + c.w.ticket) + J;
     p.npeers = npeers;
     for (int k = 0; k < npeers; ++k) p.peerL[k] = peers[k];
-    ExecMaps mp;
-    if ((rc = make_exec_maps(&mp, p, 128, 0)) != GP_OK) return rc;
     // the J trailing updates of this column were applied by the emulated contraction, outside the executor's counters
     if (cudaMemsetAsync(p.ticket, 0, sizeof(unsigned int), c.st) != cudaSuccess) return GP_ERR_CUDA;
-    oz::set_column_versions_kernel<<<(c.NB * c.nbt + 255) / 256, 256, 0, c.st>>>(p.verL, c.NB, c.nbt, J, kConsumerWarps);
-    return launch_exec<128>(p, mp, workers_for(sched_width), c.st);
+    oz::set_column_versions_kernel<<<(NB * nbt + 255) / 256, 256, 0, c.st>>>(p.verL, NB, nbt, J, kConsumerWarps);
+    return launch_exec_any(b, p, 0, workers_for(sched_width), c.st);
 }
 }  // namespace
 

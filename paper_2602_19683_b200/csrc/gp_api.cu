@@ -1266,12 +1266,14 @@ extern "C" int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sch
 namespace {
 struct MixedPredWs { size_t ticket, verV, invD, items, scale, Vt, planesL, planesV, total; };
 MixedPredWs mixed_pred_ws(int64_t n, int64_t m) {
-    const size_t NB = (size_t)(n / 128), NBm = (size_t)(m / 128);
+    // the FP64 solves run with 128-blocks or, for few test points, with 64-blocks (mixed_predict_block): counters and work
+    // items for the finer grid, inverted diagonal blocks for the coarser one
+    const size_t NB = (size_t)(n / 64), NBm = (size_t)(m / 64);
     MixedPredWs w;
     w.ticket = 0;
     w.verV = kHdrBytes;
     w.invD = align_up(w.verV + NBm * NB * sizeof(int), 256);
-    w.items = align_up(w.invD + NB * (size_t)128 * 128 * sizeof(double), 256);
+    w.items = align_up(w.invD + (size_t)n * 128 * sizeof(double), 256);
     w.scale = align_up(w.items + NBm * sizeof(Item), 256);
     w.Vt = align_up(w.scale + 256, 1024);
     w.planesL = align_up(w.Vt + (size_t)m * (size_t)n * sizeof(double), 1024);
@@ -1304,7 +1306,9 @@ int predict_mixed_impl(const double* dL, const double* dX, int64_t n, int D, con
     const MixedPredWs w = mixed_pred_ws(n, m);
     if (work_bytes < w.total) return GP_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    constexpr int b = 128;
+    // one chain per block row of V^T and tile column: m / b independent chains of tile / b dependent steps.  With few test
+    // points (c3: 32 rows of 128-blocks on 148 SMs, 0.75 ms per tile column) 64-blocks give twice the chains and cheaper steps.
+    const int b = (m / 128 <= 104) ? 64 : 128;
     const int M = (int)(n / tile), nbt = tile / b, NB = (int)(n / b), NBm = (int)(m / b);
     char* ws = (char*)dWork;
     double* Vt = (double*)(ws + w.Vt);
@@ -1379,7 +1383,8 @@ int predict_mixed_impl(const double* dL, const double* dX, int64_t n, int D, con
         cov_row_items_kernel<<<(NBm + 255) / 256, 256, 0, st>>>((uint4*)items, NBm, 0, 1, 0, (unsigned)OP_ROW_V);
         row_items_set_column_kernel<<<(NBm + 255) / 256, 256, 0, st>>>((uint4*)items, NBm, (unsigned)(P * nbt));
         p.ticket = (unsigned int*)(ws + w.ticket) + P;
-        if ((rc = launch_exec<128>(p, mp, workers_for(sched_width), st)) != GP_OK) return rc;
+        rc = b == 64 ? launch_exec<64>(p, mp, workers_for(sched_width), st) : launch_exec<128>(p, mp, workers_for(sched_width), st);
+        if (rc != GP_OK) return rc;
         if (dSigma || P + 1 < M) {              // the last column's planes only feed W
             const int64_t total = m * (tile / 4);
             const unsigned grid = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sm_count() * 16);

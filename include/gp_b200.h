@@ -262,7 +262,7 @@ int gp_ozaki_probe_stamps(long long* h_stamps8);
  *   fixed-point scale is found on the device from max_i K_ii (|L_ij| <= sqrt(K_ii)).  Everything is stream-ordered.
  *   Accuracy: the emulation truncates below 2^-56 of the scale; measured |L - L_oracle| / |L_oracle| ~ 1e-13 (tests).
  *   Same arguments and *d_info semantics as gp_cholesky_tiled; additionally tile % 128 == 0, n / tile <= 60, n <= 65536.
- *   dWork: at least gp_mixed_workspace_bytes() (dominated by the dense digit planes, 8 n^2 bytes). */
+ *   dWork: at least gp_mixed_workspace_bytes() (dominated by the dense digit planes, 7 n^2 bytes). */
 int gp_mixed_workspace_bytes(int64_t n, int tile, size_t* bytes);
 int gp_cholesky_tiled_mixed(double* dKL, int64_t n, int tile, int sched_width, int* d_info, void* dWork, size_t work_bytes,
                             void* stream);

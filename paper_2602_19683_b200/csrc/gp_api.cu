@@ -1118,13 +1118,21 @@ int mixed_ctx(int64_t n, int tile, void* dWork, size_t work_bytes, void* stream,
     c->st = (cudaStream_t)stream;
     return GP_OK;
 }
-// Block edge of the FP64 panel step of column J.  A panel is the chain of the diagonal tile (tile / b dependent POTRF -> solve ->
-// update steps: 86 us each with 128-blocks, 29 us with 64-blocks) and the solves of the block rows below it.  With many rows
-// the solves are the bulk and 128-blocks run them at the DMMA rate (64-blocks reach ~80 % of it); with few rows the chain is
-// all there is, and 64-blocks halve it: c3 panels J >= 18: 0.96 -> ~0.6 ms each.
+// Block edge of the FP64 panel step of column J.  A panel is the chain of the diagonal tile and, below it, one chain per block
+// row (the solves of a block row depend on each other, a chain keeps one SM busy): with r block rows on W workers the step takes
+// about ceil(r / W) chain times.  Measured at n = 32768, tile 1024 (ms, by 128-block rows left below the diagonal tile):
+//   128-blocks: <= 144 rows 0.90, 152-248 rows 1.45-1.57;   64-blocks: <= 72 rows 0.60, 80-144 rows 0.94, 152-216 rows 1.23-1.33,
+//   224-248 rows 1.65-1.73 -- i.e. T128 = 1 + 0.67 (waves128 - 1), T64 = 0.67 + 0.38 (waves64 - 1) in units of the 128-block chain.
+// The cheaper one is taken (c3: J = 4-12 and J >= 22 with 64-blocks: panels 37.9 -> 32 ms).  Emitting the block rows RIGHT-looking
+// (every solved block updates the blocks to its right at once, so that a row is spread over several SMs) was built and measured
+// too: 37.5 ms with 128-blocks against 36.6 ms left-looking -- the depth-one items cost more than the waves they remove.
 int mixed_panel_block(int M, int tile, int J) {
-    const int rows128 = (M - J - 1) * (tile / 128);
-    return rows128 <= 104 ? 64 : 128;
+    const int cap = g_block_edge.load(std::memory_order_relaxed);      // gp_set_block_edge: measurement override
+    if (cap == 64 || cap == 128) return cap;
+    const int rows128 = (M - J - 1) * (tile / 128), W = sm_count();
+    const int w128 = rows128 > 0 ? (rows128 + W - 1) / W : 1, w64 = rows128 > 0 ? (2 * rows128 + W - 1) / W : 1;
+    const double t128 = 1.0 + 0.67 * (w128 - 1), t64 = 0.67 + 0.38 * (w64 - 1);
+    return t64 < t128 ? 64 : 128;
 }
 
 int get_panel_schedule(int M, int nbt, int J, int b, CachedSchedule* out) {

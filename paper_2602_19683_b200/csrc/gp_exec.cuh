@@ -101,7 +101,7 @@ struct __align__(16) Job {   // 32 bytes, producer -> consumers
     double* C;             // output block (POTRF: the diagonal block of L)
     int* sig;              // version counter of the output block
     int ldc;
-    int nk;                // k-stages of kBK
+    int nk;                // k-stages of GemmCfg::kStageDepth
     int kind;
     int arg;               // POTRF: diagonal block index q; GEMM: versions the job adds to the block (>= 1)
 };
@@ -216,8 +216,11 @@ struct Producer {
             mbar_wait(&empty[stage], (uint32_t)(phase ^ 1), 2);
             char* dst = ring + (size_t)stage * Cfg::kStageBytes;
             mbar_arrive_expect_tx(&full[stage], (uint32_t)Cfg::kStageBytes);
-            tma_load_2d(dst, mA, a.x + kt * kBK, a.y, &full[stage]);
-            tma_load_2d(dst + Cfg::kOperandBytes, mB, b.x + kt * kBK, b.y, &full[stage]);
+#pragma unroll
+            for (int sub = 0; sub < Cfg::kSub; ++sub) {
+                tma_load_2d(dst + sub * Cfg::kSubBytes, mA, a.x + (kt * Cfg::kSub + sub) * kBK, a.y, &full[stage]);
+                tma_load_2d(dst + Cfg::kOperandBytes + sub * Cfg::kSubBytes, mB, b.x + (kt * Cfg::kSub + sub) * kBK, b.y, &full[stage]);
+            }
             if (++stage == kStages) { stage = 0; phase ^= 1; }
             if (kt == kpre && C != nullptr) {
 #pragma unroll 1
@@ -252,7 +255,7 @@ struct Producer {
             }
         }
         deps_done(t0);
-        const int nk = nq * BLK / kBK;
+        const int nk = nq * BLK / Cfg::kStageDepth;
         // merged tile columns: one job, one version per column.  The panels are streamed block by block (a block
         // is contiguous in the TMA view of its storage tile; a run of blocks need not be: the scheduling tile is
         // independent of the storage tile), and the C block is prefetched into L2 two blocks before the end.
@@ -261,15 +264,15 @@ struct Producer {
         if (op == OP_UPD_L) {
             double* C = blkL(gr, gc);
             push_job(C, p.verL + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
-            for (int q = q0; q < q1; ++q) stream(mapL, crdL(gr, q), mapL, crdL(gc, q), BLK / kBK, q == qpre ? C : nullptr, p.t);
+            for (int q = q0; q < q1; ++q) stream(mapL, crdL(gr, q), mapL, crdL(gc, q), BLK / Cfg::kStageDepth, q == qpre ? C : nullptr, p.t);
         } else if (op == OP_UPD_V) {
             double* C = blkV(gr, gc);
             push_job(C, p.verV + (size_t)gr * p.NB + gc, p.t, nk, JOB_GEMM_SUB, ncol);
-            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapL, crdL(gc, q), BLK / kBK, q == qpre ? C : nullptr, p.t);
+            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapL, crdL(gc, q), BLK / Cfg::kStageDepth, q == qpre ? C : nullptr, p.t);
         } else {
             double* C = blkS(gr, gc);
             push_job(C, p.verS + (size_t)gr * p.NBm + gc, (int)p.m, nk, JOB_GEMM_SUB, ncol);
-            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapV, crdV(gc, q), BLK / kBK, q == qpre ? C : nullptr, (int)p.m);
+            for (int q = q0; q < q1; ++q) stream(mapV, crdV(gr, q), mapV, crdV(gc, q), BLK / Cfg::kStageDepth, q == qpre ? C : nullptr, (int)p.m);
         }
     }
 
@@ -287,11 +290,11 @@ struct Producer {
         deps_done(t0);
         const int2 d = make_int2(0, gc * BLK);
         if (is_v) {
-            push_job(blkV(gr, gc), p.verV + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 1);
-            stream(mapV, crdV(gr, gc), mapD, d, BLK / kBK);
+            push_job(blkV(gr, gc), p.verV + (size_t)gr * p.NB + gc, p.t, BLK / Cfg::kStageDepth, JOB_GEMM_SET, 1);
+            stream(mapV, crdV(gr, gc), mapD, d, BLK / Cfg::kStageDepth);
         } else {
-            push_job(blkL(gr, gc), p.verL + (size_t)gr * p.NB + gc, p.t, BLK / kBK, JOB_GEMM_SET, 1);
-            stream(mapL, crdL(gr, gc), mapD, d, BLK / kBK);
+            push_job(blkL(gr, gc), p.verL + (size_t)gr * p.NB + gc, p.t, BLK / Cfg::kStageDepth, JOB_GEMM_SET, 1);
+            stream(mapL, crdL(gr, gc), mapD, d, BLK / Cfg::kStageDepth);
         }
     }
 

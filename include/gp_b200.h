@@ -51,7 +51,8 @@ enum {
     GP_ERR_HYPER = -4,       /* lengthscale <= 0, vertical <= 0, noise < 0, or non-finite */
     GP_ERR_WORKSPACE = -5,   /* work_bytes smaller than gp_workspace_bytes() reports */
     GP_ERR_CUDA = -6,        /* a CUDA runtime call failed (launch, memset, schedule upload) */
-    GP_ERR_MODE = -7         /* unknown layout mode */
+    GP_ERR_MODE = -7,        /* unknown layout mode */
+    GP_ERR_LIMIT = -8        /* the problem exceeds the fixed scratch of a no-allocation entry point (gp_solve_noalloc) */
 };
 
 enum { GP_SYM_LOWER = 0, GP_GENERAL = 1 };
@@ -102,6 +103,19 @@ int gp_cholesky_tiled(double* dKL, int64_t n, int tile, int sched_width, int* d_
  *   dWork/work_bytes: scratch, at least the `solve` size from gp_workspace_bytes(). */
 int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta,
              void* dWork, size_t work_bytes, void* stream);
+
+/* gp_solve for callers that cannot allocate or carry scratch (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): same arguments and results as gp_solve, but the scratch (ticket counters, beta when dBeta is NULL,
+ * the inverted diagonal blocks) lives in a file-scope `static __device__` array of the library, GP_SOLVE_NOALLOC_BYTES =
+ * 4.5 MB, which every GPU that loads the library holds until exit.  Its device address is taken once per device with
+ * cudaGetSymbolAddress.  The call allocates nothing: no cudaMalloc / cudaFree, no allocating library routine.
+ *   Limit: the scratch gp_solve would need must fit the array: n <= GP_SOLVE_NOALLOC_MAX_N = 8192 with the block edge the
+ *   library picks for such n (64 or 32); anything larger is rejected with GP_ERR_LIMIT before any work is enqueued.
+ *   Every call on a device shares the ONE array (it keeps the previous call's contents; the call clears what must start at
+ *   zero): calls that overlap on the GPU (different streams, or graph branches that run concurrently) RACE -- serialise them. */
+#define GP_SOLVE_NOALLOC_MAX_N 8192
+#define GP_SOLVE_NOALLOC_BYTES 4718592
+int gp_solve_noalloc(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta, void* stream);
 
 /* Predictive mean -- PAPER.md:70 (Eq. 2) through PAPER.md:72: y^ = K_{X^,X} alpha; steps a9-a10.
  * The cross-covariance is evaluated on the fly and never stored.

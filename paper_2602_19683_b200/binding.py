@@ -17,9 +17,9 @@ LIB_PATH = os.path.join(_HERE, "libgp_b200.so")
 
 GP_OK = 0
 GP_SYM_LOWER, GP_GENERAL = 0, 1
-ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA": -6, "MODE": -7}
+ERR = {"NULL": -1, "SIZE": -2, "TILE": -3, "HYPER": -4, "WORKSPACE": -5, "CUDA": -6, "MODE": -7, "LIMIT": -8}
 
-EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_predict_mean", "gp_predict_full_cov",
+EXPORTS = ("gp_assemble_tiles", "gp_cholesky_tiled", "gp_solve", "gp_solve_noalloc", "gp_predict_mean", "gp_predict_full_cov",
            "gp_workspace_bytes", "gp_tiles_to_dense", "gp_cholesky_task_counts", "gp_release_cached_schedules",
            "gp_block_size", "gp_strerror", "gp_pipeline_workspace_bytes", "gp_pipeline_host", "gp_pipeline_mixed_workspace_bytes", "gp_pipeline_host_mixed", "gp_fp64_peak_launch", "gp_schedule_selfcheck", "gp_exec_stats",
            "gp_contraction_bench_launch", "gp_predict_variance", "gp_log_marginal_likelihood",
@@ -71,6 +71,7 @@ def load() -> ctypes.CDLL:
     lib.gp_assemble_tiles.argtypes = [vp, i64, vp, i64, ci, gp_hyper, ci, ci, vp, vp]
     lib.gp_cholesky_tiled.argtypes = [vp, i64, ci, ci, vp, vp, sz, vp]
     lib.gp_solve.argtypes = [vp, i64, ci, vp, vp, vp, vp, sz, vp]
+    lib.gp_solve_noalloc.argtypes = [vp, i64, ci, vp, vp, vp, vp]
     lib.gp_predict_mean.argtypes = [vp, i64, ci, vp, vp, i64, gp_hyper, vp, vp]
     lib.gp_predict_full_cov.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
     lib.gp_predict_variance.argtypes = [vp, vp, i64, ci, vp, i64, gp_hyper, ci, ci, vp, vp, sz, vp]
@@ -186,6 +187,11 @@ def gp_solve(L: torch.Tensor, n: int, tile: int, y: torch.Tensor, alpha: torch.T
              work: torch.Tensor) -> None:
     _check(load().gp_solve(_ptr(L), n, tile, _ptr(y), _ptr(alpha), _ptr(beta), _ptr(work, torch.uint8), work.numel(), _stream()),
            "gp_solve")
+
+
+def gp_solve_noalloc(L: torch.Tensor, n: int, tile: int, y: torch.Tensor, alpha: torch.Tensor, beta: torch.Tensor | None = None) -> None:
+    """gp_solve on the library's static device scratch (n <= 8192): allocates nothing; calls that overlap on the GPU race."""
+    _check(load().gp_solve_noalloc(_ptr(L), n, tile, _ptr(y), _ptr(alpha), _ptr(beta), _stream()), "gp_solve_noalloc")
 
 
 def gp_predict_mean(X: torch.Tensor, alpha: torch.Tensor, Xs: torch.Tensor, h: Hyper, mean: torch.Tensor) -> None:

@@ -347,6 +347,7 @@ const char* gp_strerror(int code) {
         case GP_ERR_WORKSPACE: return "workspace too small";
         case GP_ERR_CUDA: return "CUDA runtime error";
         case GP_ERR_MODE: return "unknown layout mode";
+        case GP_ERR_LIMIT: return "problem exceeds the fixed scratch of the no-allocation entry point (gp_solve_noalloc: n <= 8192)";
         default: return "unknown error code";
     }
 }
@@ -468,6 +469,43 @@ int gp_solve(const double* dL, int64_t n, int tile, const double* dY, double* dA
     }
     if (rc != GP_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? GP_OK : GP_ERR_CUDA;
+}
+
+// ---- gp_solve without any allocation: the scratch is a static device array of the library ----------------------------------
+}  // extern "C"
+namespace {
+// In HOST code this name is only a stand-in for the symbol, not a device address: the address is taken per device with
+// cudaGetSymbolAddress (below) and that pointer is what the kernels receive.
+static __device__ __align__(256) unsigned char g_solve_noalloc_scratch[GP_SOLVE_NOALLOC_BYTES];
+void* g_solve_noalloc_ptr[kMaxDevices];          // per device, guarded by g_mu
+
+int solve_noalloc_scratch(void** out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return GP_ERR_CUDA;
+    if (dev < 0 || dev >= kMaxDevices) return GP_ERR_SIZE;
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_solve_noalloc_ptr[dev]) {
+        void* ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_solve_noalloc_scratch) != cudaSuccess || !ptr) return GP_ERR_CUDA;   // with `dev` current
+        g_solve_noalloc_ptr[dev] = ptr;
+    }
+    *out = g_solve_noalloc_ptr[dev];
+    return GP_OK;
+}
+}  // namespace
+extern "C" {
+
+int gp_solve_noalloc(const double* dL, int64_t n, int tile, const double* dY, double* dAlpha, double* dBeta, void* stream) {
+    if (!dL || !dY || !dAlpha) return GP_ERR_NULL;
+    if (n <= 0) return GP_ERR_SIZE;
+    int rc = tile_ok(n, tile);
+    if (rc != GP_OK) return rc;
+    if (n > GP_SOLVE_NOALLOC_MAX_N || solve_ws(n, pick_block(tile, n)).total > (size_t)GP_SOLVE_NOALLOC_BYTES) return GP_ERR_LIMIT;
+    void* scratch = nullptr;
+    if ((rc = solve_noalloc_scratch(&scratch)) != GP_OK) return rc;
+    // the existing path, unchanged, on the static scratch: it clears its counters and marks beta / alpha "not yet computed"
+    // itself, so the previous call's contents do not matter
+    return gp_solve(dL, n, tile, dY, dAlpha, dBeta, scratch, (size_t)GP_SOLVE_NOALLOC_BYTES, stream);
 }
 
 int gp_predict_mean(const double* dX, int64_t n, int D, const double* dAlpha, const double* dXs, int64_t m, gp_hyper h, double* dMean,

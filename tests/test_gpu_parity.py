@@ -261,6 +261,28 @@ def test_fp64_peak_probe_launches(gp):
     assert float(sink.item()) == 0.0
 
 
+@pytest.mark.parametrize("n,tile,D", [(1024, 256, 8), (384, 128, 4)])
+def test_solve_in_place_and_repeated_on_the_same_scratch(gp, n, tile, D):
+    """gp_solve publishes the pieces of beta and alpha by their VALUES (a 'not yet computed' pattern in the output vectors):
+    the header allows dAlpha == dY, and the scratch of one call may be reused by the next with other right-hand sides."""
+    X, y = nfir.nfir_features(61, n, D)
+    _, y2 = nfir.nfir_features(62, n, D)
+    h = oracle.Hyper()
+    Lo = oracle.cholesky(oracle.assemble(X, X, h, True))
+    pipe = gp.GpPipeline(n, 0, D, tile, gp.Hyper())
+    pipe.assemble(torch.from_numpy(X).cuda())
+    pipe.cholesky()
+    for rhs in (y, y2, y):
+        want = oracle.backward_subst(Lo, oracle.forward_subst(Lo, rhs))
+        buf = torch.from_numpy(rhs.copy()).cuda()             # y in, alpha out, same buffer
+        gp.gp_solve(pipe.KL, n, tile, buf, buf, None, pipe.work)
+        torch.cuda.synchronize()
+        assert relerr(buf.cpu().numpy(), want) <= TOL_ALPHA
+        pipe.solve(torch.from_numpy(rhs).cuda())              # separate buffers: the same bits
+        torch.cuda.synchronize()
+        assert torch.equal(buf, pipe.alpha)
+
+
 # ---------------------------------------------------------------- SURVEY.md 8(f) rows 1 and 4
 @pytest.mark.parametrize("n,m,D,tile", [(128, 128, 8, 32), (1024, 1024, 8, 256), (768, 256, 5, 128), (1280, 512, 16, 256)])
 def test_variance_only_and_log_marginal_likelihood(gp, n, m, D, tile):

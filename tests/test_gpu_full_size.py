@@ -137,6 +137,37 @@ def test_config4_largest_every_output_entry(gp):
     _every_output_entry(gp, nfir.CONFIGS[4])
 
 
+def _mixed_against_fp64(gp, cfg, pipe, res, X, Xs):
+    """Relative Frobenius distance of gp_cholesky_tiled_mixed's factor (lower part of the packed tiles) and of
+    gp_predict_full_cov_mixed's Sigma from the FP64 path's, computed on the device."""
+    n, m, t = cfg.n, cfg.m, cfg.tile
+    M = n // t
+    hg = gp.Hyper(cfg.lengthscale, cfg.vertical, cfg.noise)
+    diag = torch.tensor([I * (I + 1) // 2 + I for I in range(M)], device="cuda")
+
+    def lower_only(KL):                                 # the strict upper part of the diagonal tiles is unspecified (reading A8)
+        tiles = KL.view(M * (M + 1) // 2, t, t)
+        for d in diag.tolist():
+            tiles[d].tril_()
+        return KL
+
+    L64 = lower_only(pipe.KL.clone())
+    S64 = res.Sigma.clone()
+    nL, nS = float(L64.norm()), float(S64.norm())
+    dX, dXs = torch.from_numpy(X).cuda(), torch.from_numpy(Xs).cuda()
+    work = torch.empty(max(gp.gp_mixed_workspace_bytes(n, t), gp.gp_mixed_predict_workspace_bytes(n, m, t)), dtype=torch.uint8, device="cuda")
+    pipe.assemble(dX)
+    gp.gp_cholesky_tiled_mixed(pipe.KL, n, t, 0, pipe.info, work)
+    gp.gp_predict_full_cov_mixed(pipe.KL, dX, dXs, hg, t, 0, pipe.Sigma, work)
+    torch.cuda.synchronize()
+    assert int(pipe.info.item()) == 0
+    L64 -= lower_only(pipe.KL)
+    S64 -= pipe.Sigma
+    out = float(L64.norm()) / nL, float(S64.norm()) / nS
+    del L64, S64, work
+    return out
+
+
 def _every_output_entry(gp, cfg):
     n, m = cfg.n, cfg.m
     X, y, Xs = nfir.make_inputs(cfg)
@@ -144,6 +175,9 @@ def _every_output_entry(gp, cfg):
     pipe, res = _run(gp, cfg, X, y, Xs)
     L = pipe.dense_L().cpu().numpy()                    # strict upper zeroed by gp_tiles_to_dense
     alpha, mean, Sigma = res.alpha.cpu().numpy(), res.mean.cpu().numpy(), res.Sigma.cpu().numpy()
+    # the opt-in int8-emulated factorisation and covariance on the same inputs, compared ON THE DEVICE with
+    # the FP64 results that the rest of this test pins to the oracle: asserted at the end, after those have passed
+    mixed_dL, mixed_dS = _mixed_against_fp64(gp, cfg, pipe, res, X, Xs)
     del pipe, res
     torch.cuda.empty_cache()
     RB = 2048                                           # row block of the oracle's kernel matrices
@@ -193,3 +227,6 @@ def _every_output_entry(gp, cfg):
     d = np.diag(Sigma)
     assert d.min() >= 0.0 and d.max() <= cfg.vertical
     oracle.cholesky(Sigma[:1024, :1024] + 1e-12 * cfg.vertical * np.eye(1024))
+    # (8) the emulated path: L and Sigma within half of north_star's tolerances of the FP64 ones just verified
+    print(f"{cfg.name}: mixed vs FP64 path: |dL|/|L| = {mixed_dL:.2e}, |dSigma|/|Sigma| = {mixed_dS:.2e}")
+    assert mixed_dL <= 5e-11 and mixed_dS <= 5e-10
